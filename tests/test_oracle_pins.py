@@ -1,0 +1,364 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these tests touches the CUDA path.  Each pin names the passage of
+PAPER.md (or the DESIGN.md reading) it checks; see SURVEY.md 8(c) P1-P12.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1706_07413_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _golden(name):
+    out = {}
+    with open(os.path.join(GOLD, name)) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, v = line.split()
+            out[k] = float(v)
+    return out
+
+
+# ----------------------------------------------------------------- operators
+
+def test_D4_exact_on_quartics_and_parity_ghosts():
+    # "fourth order accurate finite differences": the 5-point
+    # centred first derivative is exact for polynomials up to degree 4.
+    N = 65
+    x = inputs.grid(N)
+    for deg in range(5):
+        d = oracle.D4(x ** deg, +1, +1)
+        np.testing.assert_allclose(d[2:-2], deg * x[2:-2] ** max(deg - 1, 0) if deg else 0 * x[2:-2],
+                                   rtol=0, atol=2e-12)
+    # parity ghosts (R2, R3): sin(2x) is odd about 0 and about pi/2; cos(2x) is even about both;
+    # with the right parities the derivative is 4th-order accurate up to the end points.
+    e1 = np.abs(oracle.D4(np.sin(2 * x), -1, -1) - 2 * np.cos(2 * x)).max()
+    e2 = np.abs(oracle.D4(np.cos(2 * x), +1, +1) + 2 * np.sin(2 * x)).max()
+    x2 = inputs.grid(2 * N - 1)
+    e1f = np.abs(oracle.D4(np.sin(2 * x2), -1, -1) - 2 * np.cos(2 * x2)).max()
+    assert 14 < e1 / e1f < 18 and e2 < 1e-5
+    # wrong parity must show up as an O(1/h) error at the ends
+    bad = np.abs(oracle.D4(np.cos(2 * x), -1, -1) + 2 * np.sin(2 * x)).max()
+    assert bad > 1.0
+
+
+def test_KO_annihilates_quintics_and_damps_nyquist():
+    # R6: Q is (eps/64h) times the 6th undivided difference: zero on degree<=5, and on the
+    # Nyquist mode (-1)^i it gives -(eps/h) (-1)^i, i.e. dissipative sign.
+    N = 33
+    x = inputs.grid(N); h = x[1]
+    for deg in range(6):
+        q = oracle.KO(x ** deg, 0.1, +1, +1)
+        assert np.abs(q[3:-3]).max() < 1e-9
+    ny = (-1.0) ** np.arange(N)
+    q = oracle.KO(ny, 0.1, +1, +1)   # even ghosts keep the alternation (N-1 even)
+    np.testing.assert_allclose(q, -(0.1 / h) * ny, rtol=1e-12)
+
+
+def test_cumrule_exact_for_cubics_and_sums_to_integral():
+    # R7: (h/24)[13(g_i+g_{i+1}) - (g_{i-1}+g_{i+2})] integrates cubics exactly on [x_i,x_{i+1}].
+    N = 33
+    x = inputs.grid(N)
+    for deg in range(4):
+        I = oracle.cumrule(x ** deg, +1, +1)
+        exact = (x[1:] ** (deg + 1) - x[:-1] ** (deg + 1)) / (deg + 1)
+        np.testing.assert_allclose(I[1:-1], exact[1:-1], rtol=0, atol=1e-14)
+    # with the right parity the sum over the grid is the integral to 4th order or better
+    e = []
+    for M in (33, 65, 129):
+        xm = inputs.grid(M)
+        e.append(abs(oracle.cumrule(np.sin(2 * xm), -1, -1).sum() - 1.0))
+    assert 14 < e[0] / e[1] < 18 and 14 < e[1] / e[2] < 18, e
+
+
+def test_tables_and_simpson_weights():
+    N = 129
+    tb = oracle.tables(N)
+    x = inputs.grid(N)
+    np.testing.assert_allclose(tb["sc"][:-1], np.sin(x[:-1]) * np.cos(x[:-1]), rtol=1e-14, atol=1e-17)
+    assert tb["sc"][-1] == 0.0 and tb["sc"][0] == 0.0
+    np.testing.assert_allclose(tb["T"][:-1], np.tan(x[:-1]) ** 2, rtol=1e-12)
+    np.testing.assert_allclose(tb["C"][1:-1] * tb["T"][1:-1], 1.0, rtol=1e-14)
+    assert abs(tb["w"].sum() - np.pi / 2) < 1e-14
+    # Simpson is exact for cubics
+    assert abs((tb["w"] * x ** 3).sum() - (np.pi / 2) ** 4 / 4) < 1e-13
+
+
+# --------------------------------------------------------------- P1 pure AdS
+
+@pytest.mark.parametrize("N", [17, 129])
+def test_P1_pure_AdS_is_bit_exact(N):
+    # north_star: "pure AdS (Phi=Pi=0) staying exactly A=1, delta=0".
+    z = np.zeros((2, N))
+    ev = oracle.Evolution(z, z, ko_eps=0.1)
+    assert np.all(ev.A == 1.0) and np.all(ev.delta == 0.0)
+    ev.step(1000)
+    assert np.all(ev.A == 1.0) and np.all(ev.Phi == 0.0) and np.all(ev.Pi == 0.0)
+    assert np.all(ev.delta == 0.0)
+    d = ev.diagnostics()
+    assert np.all(d["mass"] == 0.0) and np.all(d["resid"] == 0.0) and not d["collapsed"].any()
+
+
+# ----------------------------------------------------- P2, P3 closed forms
+
+def test_P2_delta_closed_form_fourth_order():
+    # eq (6)+(12): Phi=0, Pi=a cos^3 x => delta = a^2 cos^8 x / 8.
+    a = 0.7
+    errs = []
+    for N in (65, 129, 257, 513):
+        x = inputs.grid(N)
+        Pi = a * np.cos(x) ** 3; Pi[-1] = 0.0
+        d = oracle.delta_solve(np.zeros(N), Pi)
+        exact = a * a * np.cos(x) ** 8 / 8
+        errs.append(np.abs(d - exact).max())
+        assert d[-1] == 0.0 and np.all(d >= -1e-11)
+    r = np.array(errs[:-1]) / np.array(errs[1:])
+    assert np.all(r > 13) and np.all(r < 19), (errs, r)
+    assert errs[-1] < 1e-10
+
+
+def test_P3_A_small_amplitude_closed_form():
+    # eq (5) linearised about A=1, delta=0 (R11):
+    # (1-A)/a^2 -> (cos^3/sin) [x/16 + sin2x/64 - sin4x/64 - sin6x/192].
+    a = 1e-4
+    errs = []
+    for N in (65, 129, 257):
+        x = inputs.grid(N)
+        Pi = a * np.cos(x) ** 3; Pi[-1] = 0.0
+        s = oracle.set_initial(np.zeros(N), Pi)
+        A = s["A"][0]
+        xi = x[1:-1]
+        cf = (np.cos(xi) ** 3 / np.sin(xi)) * (xi / 16 + np.sin(2 * xi) / 64 - np.sin(4 * xi) / 64
+                                                - np.sin(6 * xi) / 192)
+        errs.append(np.abs((1 - A[1:-1]) / a ** 2 - cf).max())
+        assert A[0] == 1.0 and A[-1] == 1.0
+    assert errs[1] < errs[0] / 10 and errs[2] < 2e-8, errs   # O(h^4) + O(a^2) + round-off/a^2
+    # total mass of the linearised data: int sin^2 cos^4 = pi/32 (closed_forms.txt P3b)
+    d = oracle.diagnostics(s["Phi"], s["Pi"], s["A"])
+    assert abs(d["mass"][0] / a ** 2 - np.pi / 32) < 1e-7
+
+
+# ------------------------------------------------ P4 independent ODE solve
+
+def test_P4_constraints_against_adaptive_ode_solver():
+    # "solve Eq. (5) for A(x,0) and Eq. (6) for delta(x,0)".  Integrate the two
+    # ODEs exactly as printed with an adaptive 8th-order solver; the oracle's scans
+    # (integrated form R11, cumulative rule R7) must agree to O(h^4).
+    from scipy.integrate import solve_ivp
+
+    a, b = 0.9, 0.6
+
+    def Phi_f(x): return b * np.sin(x) * np.cos(x) ** 2 * np.sin(2 * x)   # odd at 0, ~rho^2... at pi/2
+    def Pi_f(x): return a * np.cos(x) ** 3 * (1 + 0.5 * np.cos(2 * x))     # even at 0, ~rho^3 at pi/2
+    def S(x): return Phi_f(x) ** 2 + Pi_f(x) ** 2
+
+    errsA, errsd = [], []
+    for N in (129, 257, 513):
+        x = inputs.grid(N)
+        Phi = Phi_f(x); Pi = Pi_f(x)
+        Phi[0] = Phi[-1] = 0.0; Pi[-1] = 0.0
+        s = oracle.set_initial(Phi, Pi)
+        # delta: integrate eq (6) from pi/2 inward
+        sol = solve_ivp(lambda t, y: [-np.sin(t) * np.cos(t) * S(t)], [np.pi / 2, 0.0], [0.0],
+                        method="DOP853", rtol=1e-13, atol=1e-16, t_eval=x[::-1])
+        d_ref = sol.y[0][::-1]
+        errsd.append(np.abs(s["delta"][0] - d_ref).max())
+        # A: integrate eq (5) outward from the regular series A = 1 - S(0) x^2/3 + O(x^4)
+        x0 = x[1]
+        # use a two-term-safe start: shoot from a much smaller x and let the solver reach x[1]
+        xs = 1e-4
+        te = x[1:-1]
+
+        def f5(t, y):
+            sn, cs = np.sin(t), np.cos(t)
+            return [(1 + 2 * sn * sn) / (sn * cs) * (1 - y[0]) - sn * cs * y[0] * S(t)]
+
+        sol = solve_ivp(f5, [xs, te[-1]], [1 - S(0.0) * xs * xs / 3], method="DOP853",
+                        rtol=1e-13, atol=1e-16, t_eval=te)
+        assert sol.success and x0 > xs
+        errsA.append(np.abs(s["A"][0][1:-1] - sol.y[0]).max())
+    rA = np.array(errsA[:-1]) / np.array(errsA[1:])
+    rd = np.array(errsd[:-1]) / np.array(errsd[1:])
+    assert np.all(rd > 12) and np.all(rA > 12), (errsA, errsd)
+    assert errsA[-1] < 2e-9 and errsd[-1] < 2e-10
+
+
+def test_P5_discrete_residual_of_eq5_converges():
+    # eq (5) as printed, differenced with an independent numpy 4th-order stencil at fixed
+    # interior x, on the oracle's A: residual -> 0 at 4th order.
+    res = []
+    for N in (129, 257, 513):
+        Phi, Pi, _ = inputs.make("cfg1", N=N)
+        Pi = Pi * 40.0                       # strong enough for a visible metric response
+        s = oracle.set_initial(Phi, Pi)
+        A, ph, pi = s["A"][0], s["Phi"][0], s["Pi"][0]
+        x = inputs.grid(N); h = x[1]
+        i = np.arange(N // 16, N - N // 16)
+        dA = (A[i - 2] - 8 * A[i - 1] + 8 * A[i + 1] - A[i + 2]) / (12 * h)
+        sn, cs = np.sin(x[i]), np.cos(x[i])
+        r = dA - ((1 + 2 * sn ** 2) / (sn * cs) * (1 - A[i]) - sn * cs * A[i] * (ph[i] ** 2 + pi[i] ** 2))
+        res.append(np.abs(r).max())
+    assert res[0] / res[1] > 10 and res[1] / res[2] > 10, res
+
+
+# -------------------------------------------- P6, P7 eigenmodes, omega = 3+2j
+
+@pytest.mark.parametrize("j", [0, 1, 2, 3])
+def test_P6_flux_operator_has_AdS_eigenmodes(j):
+    # eqs (2),(3) linearised: Phi=eps e_j', Pi=0 => Pi_dot = -omega_j^2 eps e_j,
+    # and Pi = eps e_j, Phi=0 => Phi_dot = eps e_j'.  omega_j = 3+2j (north_star; closed_forms.txt).
+    om = _golden("closed_forms.txt")[f"omega_{j}"]
+    eps = 1e-7
+    e_or, e_end = [], []
+    for N in (129, 257, 513):
+        x = inputs.grid(N)
+        e, de = inputs.eigenmode(j, x)
+        de[0] = de[-1] = 0.0
+        e[-1] = 0.0
+        kP, kQ, kA, d = oracle.rhs(eps * de, np.zeros(N), np.ones(N), 0.0)
+        err = np.abs(kQ / eps + om ** 2 * e)
+        e_or.append(err[0]); e_end.append(err[N // 4:].max())
+        kP, kQ, kA, d = oracle.rhs(np.zeros(N), eps * e, np.ones(N), 0.0)
+        assert np.abs(kP / eps - de).max() < 3e-3 * (129.0 / N) ** 4 * (1 + j) ** 5
+    # origin (l'Hopital, R4) and away from it: 4th order
+    assert 12 < e_or[0] / e_or[1] < 20 and 12 < e_or[1] / e_or[2] < 20, e_or
+    assert e_end[0] / e_end[1] > 12 and e_end[1] / e_end[2] > 12, e_end
+
+
+def test_P6_orthonormality_of_input_modes():
+    # R19: int e_j e_k tan^2 = delta_jk, checked with Simpson on a fine grid (input generator pin).
+    N = 2049
+    x = inputs.grid(N); tb = oracle.tables(N)
+    es = [inputs.eigenmode(j, x)[0] for j in range(4)]
+    for j in range(4):
+        for k in range(4):
+            v = (tb["w"][:-1] * tb["T"][:-1] * es[j][:-1] * es[k][:-1]).sum()
+            assert abs(v - (1.0 if j == k else 0.0)) < 1e-9
+
+
+@pytest.mark.parametrize("j,N", [(0, 129), (1, 129), (1, 257), (2, 257)])
+def test_P7_linear_periodicity_and_frequency(j, N):
+    # A single small-amplitude mode oscillates at omega_j = 3+2j (north_star): with Phi=eps e_j',
+    # Pi=0, phi = eps e_j cos(omega t): Phi(pi) = -Phi(0) (omega odd), Phi(2pi)=Phi(0), and the
+    # projection Pi_j(t) = int Pi e_j tan^2 = -eps omega sin(omega t) has 2*omega-1 zero
+    # crossings inside (0, 2pi) and amplitude eps*omega.
+    om = 3 + 2 * j
+    eps = 1e-5
+    x = inputs.grid(N); tb = oracle.tables(N)
+    e, de = inputs.eigenmode(j, x)
+    Phi0 = eps * de; Phi0[0] = Phi0[-1] = 0.0
+    ev = oracle.Evolution(Phi0, np.zeros(N), courant=0.25, ko_eps=0.1)
+    steps_pi = 8 * (N - 1)                     # t = pi exactly: dt = h/4 = pi/(8(N-1))
+    chunk = (N - 1) // 16
+    proj = []
+    for k in range(2 * steps_pi // chunk):
+        ev.step(chunk)
+        proj.append((tb["w"][:-1] * tb["T"][:-1] * ev.Pi[0][:-1] * e[:-1]).sum())
+        if (k + 1) * chunk == steps_pi:
+            flip = np.abs(ev.Phi[0] + Phi0).max() / np.abs(Phi0).max()
+    back = np.abs(ev.Phi[0] - Phi0).max() / np.abs(Phi0).max()
+    tol = 4e-5 * (129.0 / N) ** 3 * (om / 5.0) ** 4 + 3e-6
+    print('P7', j, N, flip, back, tol)
+    assert flip < tol and back < 2 * tol, (flip, back, tol)
+    proj = np.array(proj)
+    crossings = np.count_nonzero(np.sign(proj[:-2]) * np.sign(proj[1:-1]) < 0)
+    assert crossings == 2 * om - 1, crossings
+    assert abs(np.abs(proj).max() / (eps * om) - 1.0) < 5e-3
+    # BC invariants (P11) along the way
+    assert ev.Phi[0][0] == 0 and ev.Phi[0][-1] == 0 and ev.Pi[0][-1] == 0
+    assert ev.A[0][0] == 1 and ev.A[0][-1] == 1 and ev.delta[0][-1] == 0
+
+
+# --------------------------------- P8 self-convergence, P9 mass, constraint R
+
+def test_P8_P9_self_convergence_mass_and_residual():
+    # "solutions converge to a unique solution as the resolution is increased";
+    # mass conserved; constraint residual monitored.  Same physical time on 4 levels.
+    levels = (129, 257, 513, 1025)
+    t_steps0 = 256                            # steps on the coarsest level: t = 256*0.25*h0 = pi/4... (0.785)
+    sols, dM, R = [], [], []
+    for lv, N in enumerate(levels):
+        Pi = inputs.gaussian_Pi(N, 2.0, 0.25)
+        ev = oracle.Evolution(np.zeros((1, N)), Pi)
+        M0 = ev.diagnostics()["mass"][0]
+        ev.step(t_steps0 * 2 ** lv)
+        d = ev.diagnostics()
+        dM.append(abs(d["mass"][0] - M0) / M0); R.append(d["resid"][0])
+        st = 2 ** lv
+        sols.append([ev.Phi[0][::st], ev.Pi[0][::st], ev.A[0][::st], ev.delta[0][::st]])
+        assert ev.Phi[0][0] == 0 and ev.Phi[0][-1] == 0 and ev.Pi[0][-1] == 0      # P11
+        assert ev.A[0][0] == 1 and ev.A[0][-1] == 1
+    h0 = (np.pi / 2) / 128
+    for f, name in enumerate(["Phi", "Pi", "A", "delta"]):
+        d = [np.sqrt(h0 * ((sols[l][f] - sols[l + 1][f]) ** 2).sum()) for l in range(3)]
+        order1, order2 = np.log2(d[0] / d[1]), np.log2(d[1] / d[2])
+        assert order2 > 3.5 and order1 > 3.0, (name, d, order1, order2)
+    # Hamiltonian-constraint residual (A evolved by eq 4 vs A from eq 5): 4th order
+    assert R[1] / R[2] > 12 and R[2] / R[3] > 12, R
+    # mass drift -> 0 at least as fast as h^4, and far below the paper's 1%
+    assert dM[3] < 1e-9 and dM[1] / dM[2] > 12, dM
+
+
+def test_P10_linear_energy_of_two_mode_data():
+    # R20 + PAPER.md:83: for small amplitude M0 -> sum omega_j^2 a_j^2.
+    N = 1025
+    a_tot, ratio, th = 1e-3, 0.5, 1.1
+    Phi, Pi = inputs.two_mode(N, a_tot, ratio, th)
+    q = (3.0 / 5.0) * np.sqrt(ratio)
+    a0 = a_tot / np.sqrt(1 + q * q); a1 = q * a0
+    ev = oracle.Evolution(Phi, Pi)
+    M0 = ev.diagnostics()["mass"][0]
+    expect = 9 * a0 ** 2 * 1.0 + 25 * a1 ** 2      # cos^2+sin^2 of theta_1 sums to 1 for mode 1
+    assert abs(M0 / expect - 1) < 1e-5, (M0, expect)
+
+
+# --------------------------------------------------- survey probe cross-checks
+
+def test_survey_probe_reference_values():
+    g = _golden("survey_probe_values.txt")
+    Phi, Pi, _ = inputs.make("cfg1")
+    ev = oracle.Evolution(Phi, Pi)
+    d = ev.diagnostics()
+    assert abs(d["mass"][0] / g["M0_sigma1/16_N1025_eps1"] - 1) < 1e-11
+    assert abs(d["min_A"][0] - g["minA0_sigma1/16_N1025_eps1"]) < 1e-8
+    assert abs(ev.delta[0][0] / g["delta0_at_0_sigma1/16_N1025_eps1"] - 1) < 1e-6
+    Pi = inputs.gaussian_Pi(2049, 1.0, 0.25)
+    ev = oracle.Evolution(np.zeros_like(Pi), Pi)
+    assert abs(ev.diagnostics()["mass"][0] / g["M0_sigma1/4_N2049_eps1"] - 1) < 1e-11
+
+
+def test_P12_collapse_sanity_against_survey_probe():
+    # collapse signalled by min A -> small; thr = 2^-7 (BASELINE.json configs[1]).
+    g = _golden("survey_probe_values.txt")
+    N = 1025
+    Pi = inputs.gaussian_Pi(N, [45.0, 60.0, 20.0, 30.0], 1.0 / 16)
+    ev = oracle.Evolution(np.zeros_like(Pi), Pi, thr=2.0 ** -7, nthreads=4)
+    ev.step(10431)                                   # t = 4
+    d = ev.diagnostics()
+    assert list(d["collapsed"]) == [1, 1, 0, 0]
+    assert d["steps_done"][0] == g["collapse_step_eps45"] and d["argmin_A"][0] == g["collapse_argmin_eps45"]
+    assert d["steps_done"][1] == g["collapse_step_eps60"] and d["argmin_A"][1] == g["collapse_argmin_eps60"]
+    np.testing.assert_allclose(d["t_collapse"][:2], d["steps_done"][:2] * ev.dt, rtol=1e-15)
+    assert np.isnan(d["t_collapse"][2:]).all() and (d["steps_done"][2:] == 10431).all()
+    assert abs(d["min_A"][2] - g["minA_t4_eps20"]) < 2e-4 and abs(d["min_A"][3] - g["minA_t4_eps30"]) < 2e-4
+    # frozen members do not move when stepped again
+    A_before = ev.A[:2].copy()
+    ev.step(5)
+    assert np.array_equal(ev.A[:2], A_before) and (ev.steps_done[2:] == 10436).all()
+
+
+def test_A_resolve_period_keeps_constraint_tight():
+    # PAPER.md:81 "periodically integrating A(x,t) over space helps improve stability and
+    # accuracy" (R10): with K_A>0 the residual right after a re-solve is round-off.
+    N = 257
+    Pi = inputs.gaussian_Pi(N, 10.0, 1.0 / 8)
+    free = oracle.Evolution(np.zeros_like(Pi), Pi, K_A=0).step(512).diagnostics()
+    tight = oracle.Evolution(np.zeros_like(Pi), Pi, K_A=16).step(512).diagnostics()
+    assert tight["resid"][0] < 1e-13 and free["resid"][0] > 1e-9
+    assert abs(tight["mass"][0] / free["mass"][0] - 1) < 1e-5
