@@ -1,0 +1,143 @@
+/*
+ * adsc.h — C ABI of libadsc: batched RK4 time step of the spherically symmetric
+ * Einstein-Klein-Gordon system in AdS4 (Liebling & Khanna, arXiv:1706.07413,
+ * Sec. II; cited below as PAPER.md:<line>), on one NVIDIA B200 (sm_100a).
+ *
+ * State per ensemble member: Phi = phi', Pi = e^{delta} phi_t / A and the metric
+ * function A on the uniform grid x_i = i*h, h = (pi/2)/(N-1), i = 0..N-1
+ * (PAPER.md:39-41).  delta is not stored: it is re-integrated from Phi, Pi
+ * (eq (6)) at every Runge-Kutta stage by an on-device prefix scan,
+ * which replaces the paper's per-step host round trip.
+ *
+ * Conventions for every entry point
+ *   - "device pointer": memory of the CUDA device that was current when
+ *     adsc_bind was called; "host pointer": ordinary host memory.
+ *   - External field layout: row-major [batch][N] doubles, member b at
+ *     ptr + b*N; rows need only 8-byte alignment.
+ *   - The caller owns every buffer it passes (workspace, fields, host_out).
+ *     The library owns only the handle; it never frees caller memory and keeps
+ *     no field pointer after a call returns (the workspace pointer is kept
+ *     until adsc_destroy or the next adsc_bind).
+ *   - All work is enqueued on the stream given to adsc_bind.  Calls return
+ *     without synchronising unless stated.
+ *   - int-returning functions give ADSC_OK (0) or a negative ADSC_E* code; the
+ *     message is available from adsc_last_error.  Nothing throws or exits.
+ *   - Collapse of a member is not an error; it is reported per member.
+ *   - There is no CPU fallback: without a CUDA device every compute call
+ *     returns ADSC_ECUDA.
+ */
+#ifndef ADSC_H
+#define ADSC_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ADSC_OK       0
+#define ADSC_EINVAL  -1   /* bad argument                                        */
+#define ADSC_ESTATE  -2   /* call order (e.g. step before bind / set_initial)    */
+#define ADSC_ENOMEM  -3   /* workspace too small / host allocation failed        */
+#define ADSC_ECUDA   -4   /* CUDA runtime error; text in adsc_last_error         */
+
+/* adsc_set_option keys */
+#define ADSC_OPT_COLLAPSE_THRESHOLD 1  /* thr: member collapses when !(min_i A_i >= thr)
+                                          (PAPER.md:85).  Default 2^-7; paper uses 0.01. */
+#define ADSC_OPT_A_RESOLVE_PERIOD   2  /* K_A: every K_A steps A is replaced by the
+                                          integral of eq (5) ("periodically integrating
+                                          A").  Default 0 = never.          */
+#define ADSC_OPT_PATH               3  /* 0 auto (default), 1 force the streaming
+                                          (global-memory) kernels, 2 force the resident
+                                          (shared-memory/register) kernel; EINVAL if the
+                                          forced path cannot hold N.                    */
+#define ADSC_OPT_STEPS_PER_LAUNCH   4  /* resident path: RK4 steps per kernel launch
+                                          (default 0 = all steps of a call in one launch) */
+
+typedef struct adsc_ctx *adsc_handle;
+
+/* One record per member, filled by adsc_diagnostics (host memory). */
+typedef struct {
+    double    t;                    /* steps_done*dt (= t_collapse once collapsed)          */
+    long long steps_done;           /* RK4 steps taken by this member                       */
+    double    min_A;                /* min_i A_i of the current state (NaNs ignored)        */
+    int       argmin_A;             /* smallest i attaining min_A                           */
+    int       collapsed;            /* 1 once !(min_i A_i >= thr) was seen after a step     */
+    double    mass;                 /* M = int_0^{pi/2} tan^2 x A (Phi^2+Pi^2) dx,
+                                       composite Simpson                      */
+    double    constraint_residual;  /* max_i |A_i - A^c_i|, A^c = integral of eq (5)
+                                                                           */
+    double    t_collapse;           /* time of the step that tripped thr; NaN if none       */
+} adsc_diag;
+
+/* Create a solver for `batch` members on N grid points.
+ *   N        >= 9 and odd (Simpson needs N-1 even)
+ *   courant  dt = courant*h, 0 < courant <= 1 (method-of-lines RK4)
+ *   ko_eps   >= 0: Kreiss-Oliger coefficient of the 7-point dissipation added to the
+ *            right-hand sides of Phi and Pi (BASELINE.json configs[0]; not in the paper)
+ * Host-only; touches no device.  Returns NULL on bad arguments or host OOM. */
+adsc_handle adsc_create(int N, int batch, double courant, double ko_eps);
+
+/* Release the handle (not the workspace).  NULL is allowed. */
+int adsc_destroy(adsc_handle h);
+
+/* Bytes of device workspace adsc_bind needs (state, stage buffers, tables,
+ * per-member records).  0 if h is NULL. */
+size_t adsc_workspace_bytes(adsc_handle h);
+
+/* Attach device workspace (256-byte aligned, >= adsc_workspace_bytes) and the
+ * CUDA stream (a cudaStream_t cast to void*; NULL = legacy default stream) all
+ * later calls run on.  Builds the coefficient tables on the device.
+ * Invalidates any state previously set. */
+int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream);
+
+/* Set an option (keys above).  Allowed any time after adsc_create. */
+int adsc_set_option(adsc_handle h, int key, double value);
+
+/* Initial data: copies Phi(x,0), Pi(x,0) from device pointers
+ * [batch][N], forces Phi_0 = Phi_{N-1} = Pi_{N-1} = 0 (eqs (7),(9),(10)), integrates
+ * eq (6) for delta with delta(pi/2)=0 (eq (12)) and eq (5) for A with A(0)=A(pi/2)=1
+ * (eqs (8),(11)); resets step counters and collapse flags.  Asynchronous. */
+int adsc_set_initial(adsc_handle h, const double *d_Phi, const double *d_Pi);
+
+/* Exact resume: like adsc_set_initial but A is taken from d_A instead of being
+ * integrated (A is evolved by eq (4)).  Counters reset. */
+int adsc_set_state(adsc_handle h, const double *d_Phi, const double *d_Pi, const double *d_A);
+
+/* Advance every non-collapsed member by nsteps classical RK4 steps of
+ * eqs (2)-(4): 4th-order centred differences in flux form with parity
+ * ghosts at x=0 and x=pi/2, KO dissipation, delta re-integrated at every stage, A evolved
+ * pointwise; after each step the collapse test of PAPER.md:85.  A member that collapses
+ * is frozen at the state that tripped the threshold.  nsteps >= 0.  Asynchronous. */
+int adsc_step(adsc_handle h, long long nsteps);
+
+/* Reduce per-member diagnostics on the device, synchronise the stream and copy
+ * batch records to host_out[batch] (host pointer). */
+int adsc_diagnostics(adsc_handle h, adsc_diag *host_out);
+
+/* Copy the current fields to device pointers [batch][N]; any pointer may be NULL.
+ * d_delta is integrated from the current Phi, Pi.  Asynchronous. */
+int adsc_get_fields(adsc_handle h, double *d_Phi, double *d_Pi, double *d_A, double *d_delta);
+
+/* Convenience for host buffers (used by the end-to-end benchmark): the same as
+ * adsc_set_initial / adsc_get_fields but with HOST pointers; the library stages
+ * them through its workspace with cudaMemcpyAsync on the bound stream and, for
+ * the getter, synchronises before returning. */
+int adsc_set_initial_host(adsc_handle h, const double *h_Phi, const double *h_Pi);
+int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta);
+
+/* Number of kernels this handle has launched since adsc_bind (for gpu_launches). */
+long long adsc_launch_count(adsc_handle h);
+
+/* Which kernel family adsc_step uses for this handle: 1 streaming, 2 resident;
+ * *cluster (may be NULL) receives the CTAs per member of the resident path. */
+int adsc_path(adsc_handle h, int *cluster);
+
+/* Text of the last error on this handle (or of the last failed adsc_create if
+ * h is NULL).  Never NULL; valid until the next call on the handle. */
+const char *adsc_last_error(adsc_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ADSC_H */

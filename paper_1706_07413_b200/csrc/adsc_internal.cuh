@@ -1,0 +1,151 @@
+// adsc_internal.cuh — shared declarations of libadsc (CUDA path only; nothing here is
+// used by, or taken from, oracle/).  Notation follows include/adsc.h and DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+#include <string>
+
+#include "../../include/adsc.h"
+
+namespace adsc {
+
+constexpr int HAL = 4;            // table halo on each side (3 used by the widest stencil)
+constexpr int GEN_TILE = 1024;    // points per CTA tile of the streaming kernels
+constexpr int GEN_THREADS = 256;  // 4 points per thread
+
+// Per-member record kept on the device (copied to the host by adsc_diagnostics).
+struct MemberRec {
+    long long steps_done;
+    double t_collapse;
+    double min_A;
+    double mass;
+    double resid;
+    int argmin_A;
+    int collapsed;
+    int bad;        // streaming path: set by stage 4 / re-solve when !(A_i >= thr) for some i
+    int pad;
+};
+
+// Coefficient tables, each of length NP + 2*HAL, pointer already offset so that
+// index i in [-HAL, N-1+HAL] is valid; ghosts hold the mirrored values.
+struct Tables {
+    const double *sc;    // sin x cos x          parity (-,-), sc[0]=sc[N-1]=0
+    const double *T;     // tan^2 x              parity (+,+), T[N-1]=0 (never used as a value)
+    const double *C;     // cot^2 x              parity (+,+), C[0]=C[N-1]=0 (never used)
+    const double *c3s;   // cos^3 x / sin x      c3s[0]=c3s[N-1]=0 (never used)
+    const double *w;     // Simpson weights, 0 outside [0,N-1]
+};
+
+struct Problem {
+    int N, NP, B;
+    double h, dt, ko_eps, thr;
+};
+
+// Device pointers into the caller's workspace.
+struct Workspace {
+    double *U[3];        // state Phi, Pi, A          [B][NP]
+    double *Ua[3];       // streaming: stage state ping
+    double *Ub[3];       // streaming: stage state pong
+    double *ACC[3];      // streaming: u^n + dt/6 * partial sum
+    double *dl;          // streaming: tile-local suffix sums of I; also delta scratch
+    double *Ac;          // scratch: A from eq (5) (diagnostics)
+    double *tot;         // streaming: [B][ntiles] tile totals
+    double *carry;       // streaming: [B][ntiles] exclusive suffix of tot
+    double *stage[2];    // host staging [B][N]
+    double *tab;         // 5 tables
+    MemberRec *rec;      // [B]
+};
+
+struct Layout {
+    size_t off_U[3], off_Ua[3], off_Ub[3], off_ACC[3], off_dl, off_Ac, off_tot, off_carry,
+        off_stage[2], off_tab, off_rec, total;
+    int ntiles;
+};
+
+}  // namespace adsc
+
+struct adsc_ctx {
+    adsc::Problem pb;
+    double courant;
+    int K_A;                 // A re-solve period (0 = never)
+    int path_opt;            // ADSC_OPT_PATH
+    long long steps_per_launch;
+    int path;                // resolved: 1 streaming, 2 resident
+    int cluster;             // CTAs per member (resident)
+    int res_cfg;             // index into the resident configuration table
+    bool bound, have_state;
+    cudaStream_t stream;
+    void *ws_base;
+    adsc::Layout lay;
+    adsc::Workspace ws;
+    adsc::Tables tb;
+    long long launches;
+    long long global_step;   // steps since set_initial (lock-step over active members)
+    int dev_sms;
+    int dev_smem_optin;
+    std::string err;
+};
+
+namespace adsc {
+
+// ---- launchers implemented in the .cu files (all asynchronous on ctx->stream) -----------
+cudaError_t launch_tables(adsc_ctx *c);
+cudaError_t launch_pack(adsc_ctx *c, const double *src, int field, bool init_rec);
+cudaError_t launch_unpack(adsc_ctx *c, const double *src_internal, double *dst);
+// mode bits for launch_solve
+enum { SOLVE_WRITE_A = 1, SOLVE_DIAG = 2, SOLVE_ACTIVE_ONLY = 4 };
+cudaError_t launch_solve(adsc_ctx *c, int mode);
+cudaError_t launch_finalize(adsc_ctx *c, int inc_steps);
+cudaError_t launch_stream_step(adsc_ctx *c);                 // one RK4 step, streaming path
+cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last);  // resident path
+bool resident_select(adsc_ctx *c);                           // fills c->cluster, c->res_cfg
+const char *resident_cfg_name(int cfg);
+
+// ---- device helpers ----------------------------------------------------------------------
+#ifdef __CUDACC__
+
+// Mirror a (possibly ghost) index into [0, N-1] and return the parity sign to apply:
+// u_{-k} = p0 u_k, u_{N-1+k} = ppi u_{N-1-k}  (readings R2, R3).
+__device__ __forceinline__ int mirror(int j, int N, int p0, int ppi, double &sgn)
+{
+    sgn = 1.0;
+    if (j < 0) { j = -j; sgn = (double)p0; }
+    else if (j > N - 1) { j = 2 * (N - 1) - j; sgn = (double)ppi; }
+    return j;
+}
+
+__device__ __forceinline__ double ld_ghost(const double *__restrict__ u, int j, int N, int p0, int ppi)
+{
+    double s;
+    int k = mirror(j, N, p0, ppi, s);
+    return s * u[k];
+}
+
+// Inclusive suffix sum over the lanes of a warp: lane l gets sum_{m>=l} v_m.
+__device__ __forceinline__ double warp_suffix_incl(double v)
+{
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        double o = __shfl_down_sync(0xffffffffu, v, d);
+        if (lane + d < 32) v += o;
+    }
+    return v;
+}
+
+// Inclusive prefix sum over the lanes of a warp: lane l gets sum_{m<=l} v_m.
+__device__ __forceinline__ double warp_prefix_incl(double v)
+{
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        double o = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += o;
+    }
+    return v;
+}
+
+#endif  // __CUDACC__
+
+}  // namespace adsc
