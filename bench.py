@@ -135,3 +135,200 @@ def oracle_rate(name, N, seconds, rk4_cap=None):
     return dict(value=rate, unit=UNIT, cores=thr, kind="oracle",
                 sample=f"{B} members of {name} (N={N}) x {n} RK4 steps, {el:.1f} s, oracle/adsc_oracle.c "
                        f"gcc -O2 -ffp-contract=off, OpenMP over members"), el, n, B
+
+
+# ----------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """`--impl reference`: the oracle as it stands on the host cores, same config/metric/unit.
+    Each bench step is a bounded sample: min(B, 2 x cores) members x n RK4 steps (n sized from a
+    calibration so that warmup+steps stay within ~cpu-seconds each ... a few minutes in total)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_1706_07413_b200 import inputs
+    name = args.workload
+    N = inputs.CONFIGS[name]["N"]
+    cores = os.cpu_count() or 1
+    thr = min(cores, oracle.max_threads())
+    B = min(inputs.CONFIGS[name]["B"], 2 * thr)
+    thr = min(thr, B)
+    Phi, Pi, _ = inputs.make(name, B=B)
+    ev = oracle.Evolution(Phi, Pi, nthreads=thr)
+    t = time.perf_counter(); ev.step(2); cal = (time.perf_counter() - t) / 2
+    budget = max(1.0, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
+    n = max(1, int(budget / max(cal, 1e-9)))
+    for _ in range(args.warmup):
+        ev.step(n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ev.step(n)
+    el = time.perf_counter() - t0
+    rate = B * N * n * args.steps / el
+    sample = (f"{B} members of {name} (N={N}) x {n} RK4 steps per bench step, oracle/adsc_oracle.c "
+              f"gcc -O2 -ffp-contract=off, OpenMP over members")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic (seeded, paper_1706_07413_b200/inputs.py)",
+        "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_sampled": B, "rk4_per_step": n,
+                   "courant": 0.25, "ko_eps": 0.1},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- product arm
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_1706_07413_b200 import binding, inputs, shard
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libadsc has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    name = args.workload
+    cfg = inputs.CONFIGS[name]
+    N = cfg["N"]
+    B = args.batch or cfg["B"]              # members PER GPU (weak scaling: members are independent)
+    rk4 = args.rk4_per_step or RK4_PER_STEP[name]
+    K, W = args.steps, max(args.warmup, 0)
+
+    # Rank r evolves members [r*B, (r+1)*B) of the (tiled) seeded ensemble: no exchange step.
+    lo, hi = shard.member_range(rank, world, B * world)
+    Phi_all, Pi_all, _ = inputs.make(name, B=hi)
+    Phi_h = torch.from_numpy(np.ascontiguousarray(Phi_all[lo:hi])).pin_memory()
+    Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all[lo:hi])).pin_memory()
+    del Phi_all, Pi_all
+
+    ens = binding.Ensemble(N, B, device=dev, path=args.path)
+    path, cluster = ens.path
+    Phi_d, Pi_d = Phi_h.to(dev), Pi_h.to(dev)
+    ens.set_initial(Phi_d, Pi_d)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing: K bench steps, each one adsc_step(rk4) call
+    for _ in range(W):
+        ens.step(rk4)
+    barrier()
+    l0 = ens.launch_count
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    t0 = time.time()
+    for a, b in evs:
+        flush.fill_(1)                      # L2 flush between timed iterations (outside the events)
+        a.record()
+        ens.step(rk4)
+        b.record()
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    launches = ens.launch_count - l0
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    d = ens.diagnostics()
+    active_frac = float((d["collapsed"] == 0).mean())
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    updates = float(B) * world * N * rk4 * K
+    value = updates / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of Phi, Pi + step + D2H of the fields
+    Phi_o = torch.empty_like(Phi_h).pin_memory(); Pi_o = torch.empty_like(Phi_h).pin_memory()
+    A_o = torch.empty_like(Phi_h).pin_memory()
+    Ke = max(1, min(K, 5))
+    out = {"Phi": Phi_o, "Pi": Pi_o, "A": A_o}
+    for _ in range(1):
+        ens.set_initial(Phi_h, Pi_h); ens.step(rk4); ens.get_fields_host(delta=False, out=out)
+    barrier()
+    te0 = time.perf_counter()
+    for _ in range(Ke):
+        ens.set_initial(Phi_h, Pi_h)
+        ens.step(rk4)
+        ens.get_fields_host(delta=False, out=out)
+        dd = ens.diagnostics()
+    barrier()
+    e2e_s = time.perf_counter() - te0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = float(B) * world * N * rk4 * Ke / e2e_s
+    h2d = 2 * B * N * 8
+    d2h = 3 * B * N * 8 + B * binding.DIAG_DTYPE.itemsize
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    peaks = load_peaks()
+    per_gpu_rate = value / world
+    if path == 2:
+        peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
+        ach_tf = per_gpu_rate * SLOTS_PER_POINT_STEP * 2 / 1e12
+        roof = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": ach_tf / peak_tf, "traffic": None,
+                "kernel": "k_resident (whole RK4 steps on chip; 1 launch per adsc_step)",
+                "peak_src": f"derived: {N_SMS} SMs x {FP64_LANES_PER_SM} DFMA lanes x "
+                            f"{peaks['sm_max_mhz']:.0f} MHz x 2 flop (DESIGN.md Roofline)",
+                "algorithmic": f"{SLOTS_PER_POINT_STEP:.0f} FP64-pipe instr per point per RK4 step"}
+    else:
+        ach = per_gpu_rate * BYTES_PER_POINT_STEP / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": None,
+                "kernel": "k_stream_* (4 stage passes per RK4 step)",
+                "peak_src": f"{peaks['src']} copy bandwidth (MEASURED_PEAKS.json)",
+                "algorithmic": f"{BYTES_PER_POINT_STEP:.0f} B per point per RK4 step"}
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        cpu, _, _, _ = oracle_rate(name, N, args.cpu_seconds)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic (seeded, paper_1706_07413_b200/inputs.py)",
+        "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_per_gpu": B, "global_batch": B * world,
+                   "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1,
+                   "path": {1: "streaming", 2: "resident"}[path], "ctas_per_member": cluster,
+                   "parallelism": f"members sharded over {world} GPU(s), no collective",
+                   "l2": "flushed between timed iterations (256 MiB fill)",
+                   "active_fraction": active_frac},
+        "roofline": roof,
+        "cpu_baseline": cpu,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": Ke, "what": "adsc_set_initial_host + adsc_step + adsc_get_fields_host(Phi,Pi,A) + adsc_diagnostics"},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
