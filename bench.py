@@ -48,6 +48,7 @@ def parse():
     ap.add_argument("--rk4-per-step", type=int, default=0, help="RK4 steps per bench step (0 = workload default)")
     ap.add_argument("--batch", type=int, default=0, help="override the ensemble size (0 = workload default)")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 streaming, 2 resident")
+    ap.add_argument("--variant", type=int, default=None, help="resident kernel variant (tuning; default auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -217,7 +218,7 @@ def main():
     Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all[lo:hi])).pin_memory()
     del Phi_all, Pi_all
 
-    ens = binding.Ensemble(N, B, device=dev, path=args.path)
+    ens = binding.Ensemble(N, B, device=dev, path=args.path, resident_variant=args.variant)
     path, cluster = ens.path
     Phi_d, Pi_d = Phi_h.to(dev), Pi_h.to(dev)
     ens.set_initial(Phi_d, Pi_d)

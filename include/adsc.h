@@ -54,6 +54,11 @@ extern "C" {
 #define ADSC_OPT_STEPS_PER_LAUNCH   4  /* resident path: RK4 steps per kernel launch
                                           (default 0 = all steps of a call in one launch) */
 
+#define ADSC_OPT_RESIDENT_VARIANT    5  /* tuning: -1 auto (default) or the index of the one
+                                          resident kernel configuration (points per thread x
+                                          threads per CTA) to use; EINVAL if it cannot tile N.
+                                          Results do not depend on it beyond rounding order.  */
+
 typedef struct adsc_ctx *adsc_handle;
 
 /* One record per member, filled by adsc_diagnostics (host memory). */

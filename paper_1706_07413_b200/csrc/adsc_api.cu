@@ -84,7 +84,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->K_A = 0; c->path_opt = 0; c->steps_per_launch = 0;
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
-    c->cluster = 1; c->res_cfg = -1;
+    c->cluster = 1; c->res_cfg = -1; c->res_force = -1;
     resolve_path(c);
     return c;
 }
@@ -130,6 +130,18 @@ int adsc_set_option(adsc_handle h, int key, double value)
         if (!(value >= 0.0) || value != std::floor(value)) return fail(h, ADSC_EINVAL, "steps per launch must be a non-negative integer");
         h->steps_per_launch = (long long)value;
         return ADSC_OK;
+    case ADSC_OPT_RESIDENT_VARIANT: {
+        if (value != std::floor(value) || value < -1.0 || value > 64.0) return fail(h, ADSC_EINVAL, "bad resident variant");
+        if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_RESIDENT_VARIANT before adsc_bind");
+        const int old = h->res_force;
+        h->res_force = (int)value;
+        resolve_path(h);
+        if (h->path != 2) {
+            h->res_force = old; resolve_path(h);
+            return fail(h, ADSC_EINVAL, "this resident variant cannot hold N (or the path is forced to streaming)");
+        }
+        return ADSC_OK;
+    }
     default:
         return fail(h, ADSC_EINVAL, "unknown option key");
     }

@@ -74,6 +74,7 @@ struct adsc_ctx {
     int path;                // resolved: 1 streaming, 2 resident
     int cluster;             // CTAs per member (resident)
     int res_cfg;             // index into the resident configuration table
+    int res_force;           // ADSC_OPT_RESIDENT_VARIANT: -1 auto, else the only table entry tried
     bool bound, have_state;
     cudaStream_t stream;
     void *ws_base;
