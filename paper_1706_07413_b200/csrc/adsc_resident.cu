@@ -17,20 +17,11 @@
 #include <cooperative_groups.h>
 
 #include "adsc_internal.cuh"
+#include "adsc_resident.cuh"
 
 namespace cg = cooperative_groups;
 
 namespace adsc {
-
-struct ResParams {
-    Problem pb;
-    Tables tb;
-    double *U[3];
-    MemberRec *rec;
-    long long nsteps;
-    int check_last;   // 0: the caller re-solves A after the last step and tests collapse itself
-    int CL;
-};
 
 template <int P, int THREADS, bool ACC_REG>
 struct ResLayout {
@@ -351,19 +342,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident(const ResParams prm)
 }
 
 // ------------------------------------------------------------------ configuration table
-struct ResConfig {
-    const char *name;
-    int P, threads, seg;
-    bool acc_reg;
-    size_t smem;
-    const void *fn_single, *fn_multi;
-};
-
 #define ADSC_RES_CFG(P_, T_, ACC_)                                                        \
     { "P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, ResLayout<P_, T_, ACC_>::bytes,       \
       (const void *)k_resident<P_, T_, ACC_, false>, (const void *)k_resident<P_, T_, ACC_, true> }
 
-static const ResConfig g_cfgs[] = {
+static const ResConfig g_cfgs1[] = {
     ADSC_RES_CFG(8, 256, true),     // SEG 2048, accumulators in registers
     ADSC_RES_CFG(4, 512, false),    // SEG 2048
     ADSC_RES_CFG(4, 256, false),    // SEG 1024
@@ -371,17 +354,21 @@ static const ResConfig g_cfgs[] = {
     ADSC_RES_CFG(4, 64, false),     // SEG 256
     ADSC_RES_CFG(4, 32, false),     // SEG 128
 };
-constexpr int n_cfgs = sizeof(g_cfgs) / sizeof(g_cfgs[0]);
+constexpr int n_cfgs1 = sizeof(g_cfgs1) / sizeof(g_cfgs1[0]);
 
-const char *resident_cfg_name(int cfg) { return (cfg >= 0 && cfg < n_cfgs) ? g_cfgs[cfg].name : "none"; }
+// Variant index space: [0, n_cfgs2) generation 2 (preferred), then generation 1.
+static int n_cfgs() { return n_cfgs2 + n_cfgs1; }
+static const ResConfig &cfg_at(int k) { return k < n_cfgs2 ? g_cfgs2[k] : g_cfgs1[k - n_cfgs2]; }
+
+const char *resident_cfg_name(int cfg) { return (cfg >= 0 && cfg < n_cfgs()) ? cfg_at(cfg).name : "none"; }
 
 // Pick the widest segment that tiles N-1 with at most 8 CTAs per member (portable
 // cluster limit).  Returns false if no resident configuration holds N.
 bool resident_select(adsc_ctx *c)
 {
     const int n_act = c->pb.N - 1;
-    for (int k = 0; k < n_cfgs; ++k) {
-        const ResConfig &g = g_cfgs[k];
+    for (int k = 0; k < n_cfgs(); ++k) {
+        const ResConfig &g = cfg_at(k);
         if (c->res_force >= 0 && c->res_force != k) continue;
         if (n_act % g.seg) continue;
         const int cl = n_act / g.seg;
@@ -395,7 +382,7 @@ bool resident_select(adsc_ctx *c)
 
 cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last)
 {
-    const ResConfig &g = g_cfgs[c->res_cfg];
+    const ResConfig &g = cfg_at(c->res_cfg);
     const bool multi = c->cluster > 1;
     const void *fn = multi ? g.fn_multi : g.fn_single;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
