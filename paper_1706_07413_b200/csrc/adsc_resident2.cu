@@ -134,6 +134,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
     const double d4c = 1.0 / (12.0 * pb.h), koc = pb.ko_eps / (64.0 * pb.h);
     const double hh = 0.5 * pb.h, c25 = 25.0 * pb.h / 48.0, c12 = 0.25 * pb.h, c1 = pb.h / 48.0;
     const double thr = pb.thr;
+    const double dt_half = 0.5 * pb.dt, dt_6 = pb.dt / 6.0, dt_3 = pb.dt / 3.0;
+    const double inv12h2 = 1.0 / (12.0 * pb.h * pb.h), c_org = 1.0 / (2.0 * pb.h);
 
     // ---- load: own points to registers, u^n and tables to shared memory
     double ph[P], pi[P], a[P];
@@ -155,7 +157,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
             tSC[p * LD + col] = -2.0 * prm.tb.sc[g0 + p];
             tT[p * THREADS + tid] = prm.tb.T[g0 + p];
             tC[p * THREADS + tid] = prm.tb.C[g0 + p] * d4c;
-            if constexpr (ACC_REG) { accP[p] = 0.0; accQ[p] = 0.0; accA[p] = 0.0; }
+            if constexpr (ACC_REG) { accP[p] = ph[p]; accQ[p] = pi[p]; accA[p] = a[p]; }
+            else { accS[(0 * P + p) * THREADS + tid] = ph[p]; accS[(1 * P + p) * THREADS + tid] = pi[p]; accS[(2 * P + p) * THREADS + tid] = a[p]; }
         }
         if (lo_edge) tSC[(P - 1) * LD + 0] = -2.0 * prm.tb.sc[g0 - 1];            // odd ghost at x=0
         if (hi_edge) tSC[0 * LD + THREADS + 1] = -2.0 * prm.tb.sc[g0 + P];        // 0 at x=pi/2
@@ -219,8 +222,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
     for (long long n = 0; n < prm.nsteps; ++n) {
 #pragma unroll 1
         for (int s = 0; s < 4; ++s) {
-            const double a_next = (s == 2) ? pb.dt : 0.5 * pb.dt;
-            const double b_w = (s == 0 || s == 3) ? pb.dt / 6.0 : pb.dt / 3.0;
+            const double a_next = (s == 2) ? pb.dt : dt_half;
+            const double b_w = (s == 0 || s == 3) ? dt_6 : dt_3;
 
             // ---------------------------------------------------------------- phase 1
             double phx[P + 6], pix[P + 6];          // stage state with 3 halo points per side
@@ -241,7 +244,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
                 for (; w + 1 < NG; w += 2) { B0 += wtot[w]; B1 += wtot[w + 1]; }
                 if (w < NG) B0 += wtot[w];
                 const double B = B0 + B1;
-                const double top = last ? fo[P - 1] * (1.0 / 12.0) : 0.0;
+                const double top = last ? fo[P - 1] * (1.0 / 12.0) : 0.0;     // same expression as in finish_state
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
                     const double f_lo = (p == 0) ? fm : fo[p - 1];
@@ -256,7 +259,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
             double E[P];
             exp_near<P>(nd, E);
             // a3 fluxes; a4/a5 for A (eq 4 needs no neighbour)
-            double H[P], F[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
+            double H[P], F[P], kAv[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
             int bad = 0;
 #pragma unroll
             for (int p = 0; p < P; ++p) {
@@ -270,16 +273,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
                 if (p == P - 2) Gl2 = G;
                 double kA = (tSC[p * LD + col] * a[p]) * (G * pi[p]);    // -2 sc A G Pi
                 if (p == 0 && first) kA = 0.0;                           // A(0,t)=1, eq (8)
-                const int ui = (2 * P + p) * THREADS + tid;
-                const double bs = (s == 0) ? a[p] : un[ui];
-                double accv;
-                if constexpr (ACC_REG) accv = (s == 0) ? bs : accA[p];
-                else accv = (s == 0) ? bs : accS[ui];
-                const double accn = fma(b_w, kA, accv);
-                if (s < 3) {
-                    if constexpr (ACC_REG) accA[p] = accn; else accS[ui] = accn;
-                    a[p] = fma(a_next, kA, bs);
-                } else {
+                kAv[p] = kA;
+            }
+            // RK4 combine for A.  Invariant at the start of every step: acc == u^n == state.
+            if (s < 3) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int ui = (2 * P + p) * THREADS + tid;
+                    if constexpr (ACC_REG) accA[p] = fma(b_w, kAv[p], accA[p]);
+                    else accS[ui] = fma(b_w, kAv[p], accS[ui]);
+                    a[p] = fma(a_next, kAv[p], un[ui]);
+                }
+            } else {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int ui = (2 * P + p) * THREADS + tid;
+                    double accn;
+                    if constexpr (ACC_REG) { accn = fma(b_w, kAv[p], accA[p]); accA[p] = accn; }
+                    else { accn = fma(b_w, kAv[p], accS[ui]); accS[ui] = accn; }
                     a[p] = accn; un[ui] = accn;
                     if (!(accn >= thr)) bad = 1;
                 }
@@ -298,7 +309,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
             if (hi_edge) {
                 if (rank == CL - 1) {  // x=pi/2: H odd with H=0 there; F even with the limit of R5
                     xH[0 * LD + THREADS + 1] = 0.0; xH[1 * LD + THREADS + 1] = -H[P - 1];
-                    xF[0 * LD + THREADS + 1] = (16.0 * Gl1 - Gl2) / (12.0 * pb.h * pb.h);
+                    xF[0 * LD + THREADS + 1] = (16.0 * Gl1 - Gl2) * inv12h2;
                     xF[1 * LD + THREADS + 1] = F[P - 1];
                 } else if (MULTI) {
                     nb_hi_xH[2 * LD] = H[P - 2]; nb_hi_xH[3 * LD] = H[P - 1];
@@ -340,25 +351,31 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
                 for (int p = 0; p < P; ++p) { Hx[p + 2] = H[p]; Fx[p + 2] = F[p]; }
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
-                    double vP = fma(d4c, fma(8.0, Hx[p + 3] - Hx[p + 1], Hx[p] - Hx[p + 4]), kP[p]);
-                    double vQ = fma(tC[p * THREADS + tid], fma(8.0, Fx[p + 3] - Fx[p + 1], Fx[p] - Fx[p + 4]), kQ[p]);
+                    kP[p] = fma(d4c, fma(8.0, Hx[p + 3] - Hx[p + 1], Hx[p] - Hx[p + 4]), kP[p]);
+                    const double qq = kQ[p];
+                    kQ[p] = fma(tC[p * THREADS + tid], fma(8.0, Fx[p + 3] - Fx[p + 1], Fx[p] - Fx[p + 4]), qq);
                     if (p == 0 && first) {           // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
-                        vP = 0.0;
-                        vQ = (8.0 * G1 - G2) / (2.0 * pb.h) + kQ[0];
+                        kP[0] = 0.0;
+                        kQ[0] = fma(8.0 * G1 - G2, c_org, qq);
                     }
+                }
+            }
+            if (s < 3) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
                     const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
-                    const double bP = (s == 0) ? ph[p] : un[uP];
-                    const double bQ = (s == 0) ? pi[p] : un[uQ];
-                    double aP, aQ;
-                    if constexpr (ACC_REG) { aP = (s == 0) ? bP : accP[p]; aQ = (s == 0) ? bQ : accQ[p]; }
-                    else { aP = (s == 0) ? bP : accS[uP]; aQ = (s == 0) ? bQ : accS[uQ]; }
-                    const double nP = fma(b_w, vP, aP), nQ = fma(b_w, vQ, aQ);
-                    if (s < 3) {
-                        if constexpr (ACC_REG) { accP[p] = nP; accQ[p] = nQ; } else { accS[uP] = nP; accS[uQ] = nQ; }
-                        ph[p] = fma(a_next, vP, bP); pi[p] = fma(a_next, vQ, bQ);
-                    } else {
-                        ph[p] = nP; pi[p] = nQ; un[uP] = nP; un[uQ] = nQ;
-                    }
+                    if constexpr (ACC_REG) { accP[p] = fma(b_w, kP[p], accP[p]); accQ[p] = fma(b_w, kQ[p], accQ[p]); }
+                    else { accS[uP] = fma(b_w, kP[p], accS[uP]); accS[uQ] = fma(b_w, kQ[p], accS[uQ]); }
+                    ph[p] = fma(a_next, kP[p], un[uP]); pi[p] = fma(a_next, kQ[p], un[uQ]);
+                }
+            } else {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
+                    double nP, nQ;
+                    if constexpr (ACC_REG) { nP = fma(b_w, kP[p], accP[p]); nQ = fma(b_w, kQ[p], accQ[p]); accP[p] = nP; accQ[p] = nQ; }
+                    else { nP = fma(b_w, kP[p], accS[uP]); nQ = fma(b_w, kQ[p], accS[uQ]); accS[uP] = nP; accS[uQ] = nQ; }
+                    ph[p] = nP; pi[p] = nQ; un[uP] = nP; un[uQ] = nQ;
                 }
             }
             if (s == 3) {
@@ -405,6 +422,8 @@ const ResConfig g_cfgs2[] = {
     ADSC_RES2_CFG(4, 128, false),   // SEG 512
     ADSC_RES2_CFG(4, 64, false),    // SEG 256
     ADSC_RES2_CFG(4, 32, false),    // SEG 128
+    ADSC_RES2_CFG(4, 512, false),   // SEG 2048 (experiment: 16 warps)
+    ADSC_RES2_CFG(4, 256, false),   // SEG 1024
 };
 const int n_cfgs2 = sizeof(g_cfgs2) / sizeof(g_cfgs2[0]);
 
