@@ -50,6 +50,32 @@ struct Res2Layout {
     static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
 };
 
+// Branch-free e^x (x clamped to [-708, 709]; NaN propagates; e^0 = 1 exactly): k = rint(x log2 e),
+// r = x - k ln 2 in two pieces, Taylor polynomial of degree 13 split in two halves to shorten the
+// dependency chain (|r| <= 0.347: truncation r^14/14! < 5e-18), scaled by 2^k through the exponent field.
+__device__ __forceinline__ double exp_ref(double x)
+{
+    x = (x < -708.0) ? -708.0 : x;
+    x = (x > 709.0) ? 709.0 : x;
+    const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);
+    const int k = __double2loint(t);
+    const double kf = t - 6755399441055744.0;
+    double r = fma(kf, -6.93147180369123816490e-01, x);
+    r = fma(kf, -1.90821492927058770002e-10, r);
+    double lo = fma(r, 1.0 / 720.0, 1.0 / 120.0);
+    double hi = fma(r, 1.0 / 6227020800.0, 1.0 / 479001600.0);
+    const double r2 = r * r;
+    lo = fma(r, lo, 1.0 / 24.0);      hi = fma(r, hi, 1.0 / 39916800.0);
+    const double r3 = r2 * r, r4 = r2 * r2;
+    lo = fma(r, lo, 1.0 / 6.0);       hi = fma(r, hi, 1.0 / 3628800.0);
+    const double r7 = r4 * r3;
+    lo = fma(r, lo, 0.5);             hi = fma(r, hi, 1.0 / 362880.0);
+    lo = fma(r, lo, 1.0);             hi = fma(r, hi, 1.0 / 40320.0);
+    lo = fma(r, lo, 1.0);             hi = fma(r, hi, 1.0 / 5040.0);
+    const double e = fma(r7, hi, lo);
+    return e * __hiloint2double((k + 1023) << 20, 0);
+}
+
 // e^{x_p} for P values that lie close together: one exp at the reference x_{P-1}, the rest
 // relative to it.  exp(z) = 1 + z t(z), t = sum_{k<=5} z^k/(k+1)!; for |z| <= 2^-6 the truncation
 // is z^7/5040 < 5e-17 relative.  x = 0 gives exactly 1 (pure AdS stays bit-exact).
@@ -64,7 +90,7 @@ __device__ __forceinline__ void exp_near(const double (&x)[P], double (&E)[P])
         z[p] = x[p] - xr;
         big |= ((__double2hiint(z[p]) & 0x7fffffff) > 0x3f900000) ? 1 : 0;    // |z| > 2^-6 (or NaN)
     }
-    const double Er = exp(xr);
+    const double Er = exp_ref(xr);
     E[P - 1] = Er;
     if (!big) {
 #pragma unroll
@@ -78,7 +104,7 @@ __device__ __forceinline__ void exp_near(const double (&x)[P], double (&E)[P])
         }
     } else {
 #pragma unroll
-        for (int p = 0; p < P - 1; ++p) E[p] = exp(x[p]);
+        for (int p = 0; p < P - 1; ++p) E[p] = exp_ref(x[p]);
     }
 }
 
@@ -165,17 +191,21 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
         if (tid < 2) iflag[tid] = 0;
     }
 
-    // f' = -2 f of the own points, thread-local suffix sums s_p (s_P = top term), warp scan;
-    // publish the warp total and the state edges.  Kept across the barrier: fo, so, excl.
-    double fo[P], so[P], excl;
-    auto finish_state = [&]() {
+    // Kept across barrier S: f' = -2 f of the own points (fo), thread-local suffix sums s_p
+    // (so; s_P = top term), the exclusive warp-level suffix (excl), and the own-point part of the
+    // Kreiss-Oliger sums of the state just completed (kP, kQ).
+    double fo[P], so[P], excl, kP[P], kQ[P];
+    const double kw0 = -20.0 * koc, kw1 = 15.0 * koc, kw2 = -6.0 * koc, kw3 = koc;
+    auto kow = [&](int j) { return j == 0 ? kw0 : (j == 1 ? kw1 : (j == 2 ? kw2 : kw3)); };
+
+    // f', s of the new state; publish the state edges (stores go out before the shuffle chain).
+    auto state_sums_and_edges = [&]() {
 #pragma unroll
         for (int p = 0; p < P; ++p) fo[p] = tSC[p * LD + col] * fma(ph[p], ph[p], pi[p] * pi[p]);
         // top term of the telescoped rule: S_{N-1} = S_N = f_{N-2}/12 (f_N = -f_{N-2}, f_{N-1} = 0)
         so[P - 1] = fo[P - 1] + (last ? fo[P - 1] * (1.0 / 12.0) : 0.0);
 #pragma unroll
         for (int p = P - 2; p >= 0; --p) so[p] = so[p + 1] + fo[p];
-        // state edges first (stores), then the shuffle chain
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             xPhi[k * LD + col] = ph[k]; xPi[k * LD + col] = pi[k];
@@ -200,6 +230,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
                 for (int k = 0; k < 3; ++k) { nb_hi_xPhi[(RX - 3 + k) * LD] = ph[P - 3 + k]; nb_hi_xPi[(RX - 3 + k) * LD] = pi[P - 3 + k]; }
             }
         }
+    };
+    // a2, warp level: inclusive suffix over the lanes, publish the warp total.
+    auto warp_scan_publish = [&]() {
         const double incl = warp_suffix_incl(so[0]);
         excl = incl - so[0];
         const double wsum = __shfl_sync(0xffffffffu, incl, 0);
@@ -209,11 +242,26 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
             if (lane == 0) wtot[gw] = wsum;
         }
     };
+    // Own-point part of Q Phi, Q Pi (R6) of the state in ph, pi; the halo part is added after barrier S.
+    auto ko_own = [&]() {
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            double sP = kw0 * ph[p], sQ = kw0 * pi[p];
+#pragma unroll
+            for (int j = 1; j <= 3; ++j) {
+                if (p - j >= 0) { sP = fma(kow(j), ph[p - j], sP); sQ = fma(kow(j), pi[p - j], sQ); }
+                if (p + j < P)  { sP = fma(kow(j), ph[p + j], sP); sQ = fma(kow(j), pi[p + j], sQ); }
+            }
+            kP[p] = sP; kQ[p] = sQ;
+        }
+    };
     auto arrive = [&]() { if (MULTI) cluster_arrive(); };
     auto wait = [&]() { if (MULTI) cluster_wait(); else __syncthreads(); };
 
-    finish_state();
+    state_sums_and_edges();
+    warp_scan_publish();
     arrive();
+    ko_own();
     wait();
 
     long long n_done = 0;
@@ -225,26 +273,37 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
             const double a_next = (s == 2) ? pb.dt : dt_half;
             const double b_w = (s == 0 || s == 3) ? dt_6 : dt_3;
 
-            // ---------------------------------------------------------------- phase 1
-            double phx[P + 6], pix[P + 6];          // stage state with 3 halo points per side
+            // ---------------------------------------------------------------- phase 1 (after barrier S)
+            double hlP[3], hrP[3], hlQ[3], hrQ[3];    // 3 halo points per side of the stage state
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
-                phx[k] = xPhi[(RX - 3 + k) * LD + col - 1]; pix[k] = xPi[(RX - 3 + k) * LD + col - 1];
-                phx[P + 3 + k] = xPhi[k * LD + col + 1];    pix[P + 3 + k] = xPi[k * LD + col + 1];
+                hlP[k] = xPhi[(RX - 3 + k) * LD + col - 1]; hlQ[k] = xPi[(RX - 3 + k) * LD + col - 1];
+                hrP[k] = xPhi[k * LD + col + 1];            hrQ[k] = xPi[k * LD + col + 1];
             }
-#pragma unroll
-            for (int p = 0; p < P; ++p) { phx[p + 3] = ph[p]; pix[p + 3] = pi[p]; }
-            // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f
-            double nd[P];
+            const double scm = tSC[(P - 1) * LD + col - 1], scp = tSC[0 * LD + col + 1];
+            // a2, member level: all f' above this thread's points
+            double B0 = excl, B1 = 0.0;
             {
-                const double fm = tSC[(P - 1) * LD + col - 1] * fma(phx[2], phx[2], pix[2] * pix[2]);          // f'_{-1}
-                const double fp = tSC[0 * LD + col + 1] * fma(phx[P + 3], phx[P + 3], pix[P + 3] * pix[P + 3]); // f'_{P}
-                double B0 = excl, B1 = 0.0;           // all f' above this thread's points
                 int w = gw + 1;
                 for (; w + 1 < NG; w += 2) { B0 += wtot[w]; B1 += wtot[w + 1]; }
                 if (w < NG) B0 += wtot[w];
-                const double B = B0 + B1;
-                const double top = last ? fo[P - 1] * (1.0 / 12.0) : 0.0;     // same expression as in finish_state
+            }
+            const double B = B0 + B1;
+            // halo part of the Kreiss-Oliger sums
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+#pragma unroll
+                for (int j = 1; j <= 3; ++j) {
+                    if (p - j < 0) { kP[p] = fma(kow(j), hlP[3 + p - j], kP[p]); kQ[p] = fma(kow(j), hlQ[3 + p - j], kQ[p]); }
+                    if (p + j >= P) { kP[p] = fma(kow(j), hrP[p + j - P], kP[p]); kQ[p] = fma(kow(j), hrQ[p + j - P], kQ[p]); }
+                }
+            }
+            // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f
+            double nd[P];
+            {
+                const double fm = scm * fma(hlP[2], hlP[2], hlQ[2] * hlQ[2]);     // f'_{-1}
+                const double fp = scp * fma(hrP[0], hrP[0], hrQ[0] * hrQ[0]);     // f'_{P}
+                const double top = last ? fo[P - 1] * (1.0 / 12.0) : 0.0;         // as in state_sums_and_edges
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
                     const double f_lo = (p == 0) ? fm : fo[p - 1];
@@ -258,9 +317,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
             }
             double E[P];
             exp_near<P>(nd, E);
-            // a3 fluxes; a4/a5 for A (eq 4 needs no neighbour)
+            // a3 fluxes
             double H[P], F[P], kAv[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
-            int bad = 0;
 #pragma unroll
             for (int p = 0; p < P; ++p) {
                 const double AE = a[p] * E[p];
@@ -271,30 +329,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
                 if (p == 2) G2 = G;
                 if (p == P - 1) Gl1 = G;
                 if (p == P - 2) Gl2 = G;
-                double kA = (tSC[p * LD + col] * a[p]) * (G * pi[p]);    // -2 sc A G Pi
-                if (p == 0 && first) kA = 0.0;                           // A(0,t)=1, eq (8)
-                kAv[p] = kA;
+                kAv[p] = (tSC[p * LD + col] * a[p]) * (G * pi[p]);        // eq (4): -2 sc A G Pi
             }
-            // RK4 combine for A.  Invariant at the start of every step: acc == u^n == state.
-            if (s < 3) {
-#pragma unroll
-                for (int p = 0; p < P; ++p) {
-                    const int ui = (2 * P + p) * THREADS + tid;
-                    if constexpr (ACC_REG) accA[p] = fma(b_w, kAv[p], accA[p]);
-                    else accS[ui] = fma(b_w, kAv[p], accS[ui]);
-                    a[p] = fma(a_next, kAv[p], un[ui]);
-                }
-            } else {
-#pragma unroll
-                for (int p = 0; p < P; ++p) {
-                    const int ui = (2 * P + p) * THREADS + tid;
-                    double accn;
-                    if constexpr (ACC_REG) { accn = fma(b_w, kAv[p], accA[p]); accA[p] = accn; }
-                    else { accn = fma(b_w, kAv[p], accS[ui]); accS[ui] = accn; }
-                    a[p] = accn; un[ui] = accn;
-                    if (!(accn >= thr)) bad = 1;
-                }
-            }
+            if (first) kAv[0] = 0.0;                                      // A(0,t)=1, eq (8)
             // publish flux edges
             xH[0 * LD + col] = H[0]; xH[1 * LD + col] = H[1]; xH[2 * LD + col] = H[P - 2]; xH[3 * LD + col] = H[P - 1];
             xF[0 * LD + col] = F[0]; xF[1 * LD + col] = F[1]; xF[2 * LD + col] = F[P - 2]; xF[3 * LD + col] = F[P - 1];
@@ -316,56 +353,71 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
                     nb_hi_xF[2 * LD] = F[P - 2]; nb_hi_xF[3 * LD] = F[P - 1];
                 }
             }
-            const int par = (int)(n & 1);
-            if (MULTI && s == 3 && bad) {
-                for (int r = 0; r < CL; ++r) cluster.map_shared_rank(iflag, r)[par] = 1;
-            }
             arrive();                                                     // barrier F
 
-            // ---------------------------------------------------------------- phase 2
-            // Kreiss-Oliger terms and the interior differences need no flux halo: before the wait.
-            double kP[P], kQ[P];
-#pragma unroll
-            for (int p = 0; p < P; ++p) {
-                double t = fma(-6.0, phx[p + 1] + phx[p + 5], phx[p] + phx[p + 6]);
-                t = fma(15.0, phx[p + 2] + phx[p + 4], t);
-                kP[p] = koc * fma(-20.0, phx[p + 3], t);
-                double u = fma(-6.0, pix[p + 1] + pix[p + 5], pix[p] + pix[p + 6]);
-                u = fma(15.0, pix[p + 2] + pix[p + 4], u);
-                kQ[p] = koc * fma(-20.0, pix[p + 3], u);
-            }
-            int any = 0;
-            if (MULTI) {
-                wait();
-                if (s == 3) { any = iflag[par]; if (tid == 0) iflag[par ^ 1] = 0; }
-            } else {
-                if (s == 3) any = __syncthreads_or(bad); else __syncthreads();
-            }
-            {
-                double Hx[P + 4], Fx[P + 4];
-                Hx[0] = xH[2 * LD + col - 1]; Hx[1] = xH[3 * LD + col - 1];
-                Fx[0] = xF[2 * LD + col - 1]; Fx[1] = xF[3 * LD + col - 1];
-                Hx[P + 2] = xH[0 * LD + col + 1]; Hx[P + 3] = xH[1 * LD + col + 1];
-                Fx[P + 2] = xF[0 * LD + col + 1]; Fx[P + 3] = xF[1 * LD + col + 1];
-#pragma unroll
-                for (int p = 0; p < P; ++p) { Hx[p + 2] = H[p]; Fx[p + 2] = F[p]; }
+            // ---------------------------------------------------------------- between arrive and wait
+            // a4/a5 for A (eq 4 needs no neighbour).  Invariant at the start of every step: acc == u^n == state.
+            int bad = 0;
+            if (s < 3) {
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
-                    kP[p] = fma(d4c, fma(8.0, Hx[p + 3] - Hx[p + 1], Hx[p] - Hx[p + 4]), kP[p]);
-                    const double qq = kQ[p];
-                    kQ[p] = fma(tC[p * THREADS + tid], fma(8.0, Fx[p + 3] - Fx[p + 1], Fx[p] - Fx[p + 4]), qq);
-                    if (p == 0 && first) {           // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
-                        kP[0] = 0.0;
-                        kQ[0] = fma(8.0 * G1 - G2, c_org, qq);
-                    }
+                    const int ui = (2 * P + p) * THREADS + tid;
+                    if constexpr (ACC_REG) accA[p] = fma(b_w, kAv[p], accA[p]);
+                    else accS[ui] = fma(b_w, kAv[p], accS[ui]);
+                    a[p] = fma(a_next, kAv[p], un[ui]);
+                }
+            } else {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int ui = (2 * P + p) * THREADS + tid;
+                    double accn;
+                    if constexpr (ACC_REG) { accn = fma(b_w, kAv[p], accA[p]); accA[p] = accn; }
+                    else { accn = fma(b_w, kAv[p], accS[ui]); accS[ui] = accn; }
+                    a[p] = accn; un[ui] = accn;
+                    if (!(accn >= thr)) bad = 1;
                 }
             }
+            // interior centred differences (own fluxes only)
+            double dH[P], dF[P];
+#pragma unroll
+            for (int p = 2; p < P - 2; ++p) {
+                dH[p] = fma(8.0, H[p + 1] - H[p - 1], H[p - 2] - H[p + 2]);
+                dF[p] = fma(8.0, F[p + 1] - F[p - 1], F[p - 2] - F[p + 2]);
+            }
+            wait();                                                       // barrier F
+
+            // ---------------------------------------------------------------- phase 2
+            {
+                const double Hm2 = xH[2 * LD + col - 1], Hm1 = xH[3 * LD + col - 1];
+                const double Fm2 = xF[2 * LD + col - 1], Fm1 = xF[3 * LD + col - 1];
+                const double Hp0 = xH[0 * LD + col + 1], Hp1 = xH[1 * LD + col + 1];
+                const double Fp0 = xF[0 * LD + col + 1], Fp1 = xF[1 * LD + col + 1];
+                dH[0] = fma(8.0, H[1] - Hm1, Hm2 - H[2]);
+                dF[0] = fma(8.0, F[1] - Fm1, Fm2 - F[2]);
+                dH[1] = fma(8.0, H[2] - H[0], Hm1 - H[3]);
+                dF[1] = fma(8.0, F[2] - F[0], Fm1 - F[3]);
+                dH[P - 2] = fma(8.0, H[P - 1] - H[P - 3], H[P - 4] - Hp0);
+                dF[P - 2] = fma(8.0, F[P - 1] - F[P - 3], F[P - 4] - Fp0);
+                dH[P - 1] = fma(8.0, Hp0 - H[P - 2], H[P - 3] - Hp1);
+                dF[P - 1] = fma(8.0, Fp0 - F[P - 2], F[P - 3] - Fp1);
+            }
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                const double qq = kQ[p];
+                kP[p] = fma(d4c, dH[p], kP[p]);
+                kQ[p] = fma(tC[p * THREADS + tid], dF[p], qq);
+                if (p == 0 && first) {           // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
+                    kP[0] = 0.0;
+                    kQ[0] = fma(8.0 * G1 - G2, c_org, qq);
+                }
+            }
+            // a5: new stage state first (the scan needs it), accumulators after the shuffle chain started
+            double kPs[P], kQs[P];
             if (s < 3) {
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
                     const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
-                    if constexpr (ACC_REG) { accP[p] = fma(b_w, kP[p], accP[p]); accQ[p] = fma(b_w, kQ[p], accQ[p]); }
-                    else { accS[uP] = fma(b_w, kP[p], accS[uP]); accS[uQ] = fma(b_w, kQ[p], accS[uQ]); }
+                    kPs[p] = kP[p]; kQs[p] = kQ[p];
                     ph[p] = fma(a_next, kP[p], un[uP]); pi[p] = fma(a_next, kQ[p], un[uQ]);
                 }
             } else {
@@ -378,14 +430,38 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
                     ph[p] = nP; pi[p] = nQ; un[uP] = nP; un[uQ] = nQ;
                 }
             }
-            if (s == 3) {
-                n_done = n + 1;
-                if (any && (prm.check_last || n + 1 < prm.nsteps)) collapsed = 1;   // a6
-                if (collapsed || n + 1 == prm.nsteps) break;                        // uniform over the cluster
+            state_sums_and_edges();
+            warp_scan_publish();
+            const int par = (int)(n & 1);
+            if (MULTI && s == 3 && bad) {
+                for (int r = 0; r < CL; ++r) cluster.map_shared_rank(iflag, r)[par] = 1;
             }
-            finish_state();
             arrive();                                                     // barrier S
-            wait();
+            if (s < 3) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
+                    if constexpr (ACC_REG) { accP[p] = fma(b_w, kPs[p], accP[p]); accQ[p] = fma(b_w, kQs[p], accQ[p]); }
+                    else { accS[uP] = fma(b_w, kPs[p], accS[uP]); accS[uQ] = fma(b_w, kQs[p], accS[uQ]); }
+                }
+            }
+            ko_own();                                                     // for the next stage
+            if (s == 3) {
+                // a6: collapse test of PAPER.md:85 on A^{n+1}, folded into barrier S of stage 4
+                int any;
+                if (MULTI) {
+                    wait();
+                    any = iflag[par];
+                    if (tid == 0) iflag[par ^ 1] = 0;
+                } else {
+                    any = __syncthreads_or(bad);
+                }
+                n_done = n + 1;
+                if (any && (prm.check_last || n + 1 < prm.nsteps)) collapsed = 1;
+                if (collapsed) break;                                     // uniform over the cluster
+            } else {
+                wait();
+            }
         }
         if (collapsed) break;
     }
