@@ -343,8 +343,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident(const ResParams prm)
 
 // ------------------------------------------------------------------ configuration table
 #define ADSC_RES_CFG(P_, T_, ACC_)                                                        \
-    { "P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, ResLayout<P_, T_, ACC_>::bytes,       \
-      (const void *)k_resident<P_, T_, ACC_, false>, (const void *)k_resident<P_, T_, ACC_, true> }
+    { "P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, ResLayout<P_, T_, ACC_>::bytes, true, \
+      { (const void *)k_resident<P_, T_, ACC_, false>, (const void *)k_resident<P_, T_, ACC_, true>,       \
+        (const void *)k_resident<P_, T_, ACC_, true>, (const void *)k_resident<P_, T_, ACC_, true> } }
 
 static const ResConfig g_cfgs1[] = {
     ADSC_RES_CFG(8, 256, true),     // SEG 2048, accumulators in registers
@@ -356,9 +357,20 @@ static const ResConfig g_cfgs1[] = {
 };
 constexpr int n_cfgs1 = sizeof(g_cfgs1) / sizeof(g_cfgs1[0]);
 
-// Variant index space: [0, n_cfgs2) generation 2 (preferred), then generation 1.
-static int n_cfgs() { return n_cfgs2 + n_cfgs1; }
-static const ResConfig &cfg_at(int k) { return k < n_cfgs2 ? g_cfgs2[k] : g_cfgs1[k - n_cfgs2]; }
+// Variant index space: generation 3 (preferred), then generation 2, then generation 1.
+static int n_cfgs() { return n_cfgs3 + n_cfgs2 + n_cfgs1; }
+static const ResConfig &cfg_at(int k)
+{
+    if (k < n_cfgs3) return g_cfgs3[k];
+    k -= n_cfgs3;
+    return k < n_cfgs2 ? g_cfgs2[k] : g_cfgs1[k - n_cfgs2];
+}
+static const void *fn_for(const ResConfig &g, int cl)
+{
+    if (cl == 1) return g.fn[0];
+    if (g.any_cl) return g.fn[1];
+    return cl == 2 ? g.fn[1] : cl == 4 ? g.fn[2] : cl == 8 ? g.fn[3] : nullptr;
+}
 
 const char *resident_cfg_name(int cfg) { return (cfg >= 0 && cfg < n_cfgs()) ? cfg_at(cfg).name : "none"; }
 
@@ -373,6 +385,7 @@ bool resident_select(adsc_ctx *c)
         if (n_act % g.seg) continue;
         const int cl = n_act / g.seg;
         if (cl < 1 || cl > 8) continue;
+        if (!fn_for(g, cl)) continue;
         if (c->dev_smem_optin > 0 && g.smem > (size_t)c->dev_smem_optin) continue;
         c->res_cfg = k; c->cluster = cl;
         return true;
@@ -383,14 +396,24 @@ bool resident_select(adsc_ctx *c)
 cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last)
 {
     const ResConfig &g = cfg_at(c->res_cfg);
-    const bool multi = c->cluster > 1;
-    const void *fn = multi ? g.fn_multi : g.fn_single;
+    const void *fn = fn_for(g, c->cluster);
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
     if (e != cudaSuccess) return e;
     ResParams prm;
     prm.pb = c->pb; prm.tb = c->tb;
     for (int v = 0; v < 3; ++v) prm.U[v] = c->ws.U[v];
     prm.rec = c->ws.rec; prm.nsteps = nsteps; prm.check_last = check_last; prm.CL = c->cluster;
+    {
+        const double h = c->pb.h, dt = c->pb.dt, koc = c->pb.ko_eps / (64.0 * h);
+        ResConsts &k = prm.k;
+        k.d4c = 1.0 / (12.0 * h);
+        k.kw[0] = -20.0 * koc; k.kw[1] = 15.0 * koc; k.kw[2] = -6.0 * koc; k.kw[3] = koc;
+        k.hh = 0.5 * h; k.c25 = 25.0 * h / 48.0; k.c12 = 0.25 * h; k.c1 = h / 48.0;
+        k.inv12h2 = 1.0 / (12.0 * h * h); k.c_org = 1.0 / (2.0 * h);
+        k.a_next[0] = 0.5 * dt; k.a_next[1] = 0.5 * dt; k.a_next[2] = dt; k.a_next[3] = 0.0;
+        k.b_w[0] = dt / 6.0; k.b_w[1] = dt / 3.0; k.b_w[2] = dt / 3.0; k.b_w[3] = dt / 6.0;
+        k.thr = c->pb.thr;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(c->pb.B * c->cluster), 1, 1);
     cfg.blockDim = dim3((unsigned)g.threads, 1, 1);

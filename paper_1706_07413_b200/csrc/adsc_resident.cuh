@@ -4,6 +4,21 @@
 
 namespace adsc {
 
+// Scalars derived from (h, dt, ko_eps, thr) on the host once per launch.  They sit in the kernel
+// parameter (constant) bank, so fp64 instructions take them as c[][] operands and no register
+// holds them (generation 3; generations 1 and 2 derive them in the kernel).
+struct ResConsts {
+    double d4c;             // 1/(12 h)                      D4 weight
+    double kw[4];           // eps_KO/(64 h) * {-20, 15, -6, 1}   KO weights by distance
+    double hh;              // h/2            } telescoped delta rule for f' = -2 f
+    double c25, c12, c1;    // 25h/48, h/4, h/48
+    double inv12h2;         // 1/(12 h^2)     boundary flux limit (R5)
+    double c_org;           // 1/(2 h)        origin l'Hopital (R4)
+    double a_next[4];       // dt/2, dt/2, dt, 0      stage-state weights
+    double b_w[4];          // dt/6, dt/3, dt/3, dt/6 accumulator weights
+    double thr;
+};
+
 struct ResParams {
     Problem pb;
     Tables tb;
@@ -12,19 +27,25 @@ struct ResParams {
     long long nsteps;
     int check_last;   // 0: the caller re-solves A after the last step and tests collapse itself
     int CL;
+    ResConsts k;
 };
 
 // One compiled (points per thread, threads per CTA) configuration of a resident kernel.
+// fn[j] is the kernel for a cluster of 2^j CTAs per member (nullptr: not available); if any_cl,
+// fn[1] takes the cluster size at run time and serves every size 2..8.
 struct ResConfig {
     const char *name;
     int P, threads, seg;
     bool acc_reg;
     size_t smem;
-    const void *fn_single, *fn_multi;
+    bool any_cl;
+    const void *fn[4];
 };
 
-// generation-2 table (adsc_resident2.cu)
+// generation-2 table (adsc_resident2.cu), generation-3 table (adsc_resident3.cu)
 extern const ResConfig g_cfgs2[];
 extern const int n_cfgs2;
+extern const ResConfig g_cfgs3[];
+extern const int n_cfgs3;
 
 }  // namespace adsc

@@ -488,8 +488,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_resident2(const ResParams prm)
 
 // ------------------------------------------------------------------ configuration table
 #define ADSC_RES2_CFG(P_, T_, ACC_)                                                         \
-    { "v2P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res2Layout<P_, T_, ACC_>::bytes,       \
-      (const void *)k_resident2<P_, T_, ACC_, false>, (const void *)k_resident2<P_, T_, ACC_, true> }
+    { "v2P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res2Layout<P_, T_, ACC_>::bytes, true, \
+      { (const void *)k_resident2<P_, T_, ACC_, false>, (const void *)k_resident2<P_, T_, ACC_, true>,     \
+        (const void *)k_resident2<P_, T_, ACC_, true>, (const void *)k_resident2<P_, T_, ACC_, true> } }
 
 const ResConfig g_cfgs2[] = {
     ADSC_RES2_CFG(8, 256, true),    // SEG 2048, accumulators in registers

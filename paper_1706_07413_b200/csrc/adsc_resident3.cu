@@ -1,0 +1,584 @@
+// adsc_resident3.cu — resident RK4 kernel, third generation ("v3"): one ensemble member per CTA
+// (or per cluster of CL CTAs), the whole state on chip across all RK stages and steps.
+//
+// Arithmetic per stage is that of adsc_resident2.cu (telescoped delta rule, two synchronisation
+// points per RK stage, near-exp).  What changed, and why (profiles/r01_v2_resident.md):
+//   * Synchronisation is point-to-point.  Every sync point is an mbarrier in each CTA's shared memory:
+//     one elected lane per warp arrives on it (split arrive / wait, so the independent arithmetic
+//     placed between them overlaps the skew between warps also inside ONE CTA), and data for other
+//     CTAs of the cluster travels by st.async straight into the consumer's shared memory, completing
+//     transaction bytes on the consumer's mbarrier.  No barrier.cluster and no cluster-scope fence in the
+//     loop: the v2 cluster kernel spent 0.75 stall cycles per issued instruction in `membar` and
+//     ~490 clk per cluster barrier.
+//   * All scalars derived from h, dt, eps_KO sit in the kernel parameter bank (ResConsts) and the exp
+//     coefficients in __constant__ memory, so fp64 instructions take them as c[][] operands: v2
+//     re-materialised ~70 64-bit immediates per thread and stage with IMAD.MOV (8.7 % of all
+//     instructions) and had no register to spare.
+//   * The member-level scan step is a branch-free, fully unrolled, predicated sum of the published warp
+//     totals (two dependent-add chains) instead of a loop of dependent shared-memory loads.
+//   * The cluster size is a template parameter (1, 2, 4, 8).
+//
+// Per RK stage (equations PAPER.md:43-53 eqs (2)-(6); boundary conditions PAPER.md:59-75):
+//   phase 1  (after sync S: neighbours' Phi, Pi edges + warp totals of f)  delta, E = e^{-delta},
+//            fluxes G, H, F, eq (4) for A with its RK combine, publish H, F edges            -> sync F
+//   phase 2  Kreiss-Oliger Q Phi, Q Pi and interior D4 (before the wait), edge D4, RK combine for
+//            Phi, Pi, collapse test (stage 4), f of the NEW state, thread/warp scan,
+//            publish Phi, Pi edges + warp totals                                             -> sync S
+#include "adsc_internal.cuh"
+#include "adsc_resident.cuh"
+
+namespace adsc {
+
+template <int P, int THREADS, bool ACC_REG, int CL>
+struct Res3Layout {
+    static constexpr int SEG = P * THREADS;
+    static constexpr int LD = THREADS + 2;          // halo column on each side
+    static constexpr int NW = THREADS / 32;
+    static constexpr int NG = NW * CL;              // warps per member
+    static constexpr int RX = (P < 6) ? P : 6;      // rows of the state exchange buffers
+    static constexpr int o_xPhi = 0;
+    static constexpr int o_xPi = o_xPhi + RX * LD;
+    static constexpr int o_xH = o_xPi + RX * LD;
+    static constexpr int o_xF = o_xH + 4 * LD;
+    static constexpr int o_tSC = o_xF + 4 * LD;      // -2 sin x cos x, [P][LD] with halo columns
+    static constexpr int o_tT = o_tSC + P * LD;      // tan^2 x
+    static constexpr int o_tC = o_tT + P * THREADS;  // cot^2 x / (12 h)
+    static constexpr int o_un = o_tC + P * THREADS;
+    static constexpr int o_acc = o_un + 3 * P * THREADS;
+    static constexpr int o_wt = o_acc + (ACC_REG ? 0 : 3 * P * THREADS);   // [2][NG] {total, flag}
+    static constexpr int o_mbar = o_wt + 2 * NG * 2;                       // mbS[0], mbS[1], mbF, pad
+    static constexpr int n_doubles = o_mbar + 4;
+    static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
+    static_assert(o_wt % 2 == 0, "warp-total slots must be 16-byte aligned");
+};
+
+// exp coefficients (read as constant-bank operands)
+__constant__ double c_exp[18] = {
+    1.4426950408889634074,            // 0  log2 e
+    6755399441055744.0,               // 1  1.5 * 2^52 (round-to-nearest-integer shift)
+    -6.93147180369123816490e-01,      // 2  -ln2 (high part)
+    -1.90821492927058770002e-10,      // 3  -ln2 (low part)
+    1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0, 1.0 / 40320.0,   // 4..10: 1/k!, k=2..8
+    1.0 / 362880.0, 1.0 / 3628800.0, 1.0 / 39916800.0, 1.0 / 479001600.0, 1.0 / 6227020800.0,  // 11..15: k=9..13
+    -708.0, 709.0                     // 16, 17 clamps
+};
+
+// Branch-free e^x (x clamped to [-708, 709]; NaN propagates; e^0 = 1 exactly): k = rint(x log2 e),
+// r = x - k ln 2 in two pieces, Taylor polynomial of degree 13 split in two halves to shorten the
+// dependency chain (|r| <= 0.347: truncation r^14/14! < 5e-18), scaled by 2^k through the exponent field.
+__device__ __forceinline__ double exp3_ref(double x)
+{
+    x = (x < c_exp[16]) ? c_exp[16] : x;
+    x = (x > c_exp[17]) ? c_exp[17] : x;
+    const double t = fma(x, c_exp[0], c_exp[1]);
+    const int k = __double2loint(t);
+    const double kf = t - c_exp[1];
+    double r = fma(kf, c_exp[2], x);
+    r = fma(kf, c_exp[3], r);
+    double lo = fma(r, c_exp[8], c_exp[7]);
+    double hi = fma(r, c_exp[15], c_exp[14]);
+    const double r2 = r * r;
+    lo = fma(r, lo, c_exp[6]);        hi = fma(r, hi, c_exp[13]);
+    const double r3 = r2 * r, r4 = r2 * r2;
+    lo = fma(r, lo, c_exp[5]);        hi = fma(r, hi, c_exp[12]);
+    const double r7 = r4 * r3;
+    lo = fma(r, lo, c_exp[4]);        hi = fma(r, hi, c_exp[11]);
+    lo = fma(r, lo, 1.0);             hi = fma(r, hi, c_exp[10]);
+    lo = fma(r, lo, 1.0);             hi = fma(r, hi, c_exp[9]);
+    const double e = fma(r7, hi, lo);
+    return e * __hiloint2double((k + 1023) << 20, 0);
+}
+
+// e^{x_p} for P values that lie close together: one exp at the reference x_{P-1}, the rest
+// relative to it.  exp(z) = 1 + z t(z), t = sum_{k<=5} z^k/(k+1)!; for |z| <= 2^-6 the truncation
+// is z^7/5040 < 5e-17 relative.  x = 0 gives exactly 1 (pure AdS stays bit-exact).
+template <int P>
+__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P])
+{
+    const double xr = x[P - 1];
+    double z[P];
+    int big = 0;
+#pragma unroll
+    for (int p = 0; p < P - 1; ++p) {
+        z[p] = x[p] - xr;
+        big |= ((__double2hiint(z[p]) & 0x7fffffff) > 0x3f900000) ? 1 : 0;    // |z| > 2^-6 (or NaN)
+    }
+    const double Er = exp3_ref(xr);
+    E[P - 1] = Er;
+    if (!big) {
+#pragma unroll
+        for (int p = 0; p < P - 1; ++p) {
+            double t = fma(z[p], c_exp[8], c_exp[7]);
+            t = fma(z[p], t, c_exp[6]);
+            t = fma(z[p], t, c_exp[5]);
+            t = fma(z[p], t, c_exp[4]);
+            t = fma(z[p], t, 1.0);
+            E[p] = fma(Er * z[p], t, Er);
+        }
+    } else {
+#pragma unroll
+        for (int p = 0; p < P - 1; ++p) E[p] = exp3_ref(x[p]);
+    }
+}
+
+// ---- mbarrier / cluster primitives (PTX; sm_90+)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t cluster_rank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t map_rank(uint32_t addr, int rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_init(uint32_t mb, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mb), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t mb)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(mb) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t mb, uint32_t bytes)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(mb), "r"(bytes) : "memory");
+}
+template <bool CLUSTER_SCOPE>
+__device__ __forceinline__ void mbar_wait(uint32_t mb, uint32_t parity)
+{
+    if (CLUSTER_SCOPE)
+        asm volatile("{\n\t.reg .pred p;\n\tLAB_WAIT:\n\t"
+                     "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+                     "@p bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(mb), "r"(parity) : "memory");
+    else
+        asm volatile("{\n\t.reg .pred p;\n\tLAB_WAIT:\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+                     "@p bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(mb), "r"(parity) : "memory");
+}
+// Remote store into a peer CTA's shared memory that completes 8 (16) transaction bytes on the peer's mbarrier.
+__device__ __forceinline__ void st_async_f64(uint32_t dst_cluster, double v, uint32_t mbar_cluster)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];"
+                 ::"r"(dst_cluster), "l"(__double_as_longlong(v)), "r"(mbar_cluster) : "memory");
+}
+__device__ __forceinline__ void st_async_f64x2(uint32_t dst_cluster, double v0, double v1, uint32_t mbar_cluster)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];"
+                 ::"r"(dst_cluster), "l"(__double_as_longlong(v0)), "l"(__double_as_longlong(v1)), "r"(mbar_cluster) : "memory");
+}
+
+template <int P, int THREADS, bool ACC_REG, int CL>
+__global__ void __launch_bounds__(THREADS, 1) k_resident3(const __grid_constant__ ResParams prm)
+{
+    using L = Res3Layout<P, THREADS, ACC_REG, CL>;
+    constexpr bool MULTI = CL > 1;
+    constexpr int LD = L::LD, NW = L::NW, NG = L::NG, SEG = L::SEG, RX = L::RX;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(16) double smem[];
+    double *xPhi = smem + L::o_xPhi, *xPi = smem + L::o_xPi, *xH = smem + L::o_xH, *xF = smem + L::o_xF;
+    double *tSC = smem + L::o_tSC, *tT = smem + L::o_tT, *tC = smem + L::o_tC;
+    double *un = smem + L::o_un, *accS = smem + L::o_acc;
+    double2 *wt = reinterpret_cast<double2 *>(smem + L::o_wt);
+
+    const int rank = MULTI ? (int)cluster_rank() : 0;
+    const int b = blockIdx.x / CL;
+    MemberRec *rec = prm.rec + b;
+    if (rec->collapsed || prm.nsteps <= 0) return;      // uniform over the cluster
+
+    const Problem &pb = prm.pb;
+    const ResConsts &K = prm.k;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, col = tid + 1;
+    const int g0 = rank * SEG + tid * P;                 // first owned grid index
+    const bool lo_edge = (tid == 0), hi_edge = (tid == THREADS - 1);
+    const bool first = lo_edge && rank == 0;             // owns i = 0
+    const bool last = hi_edge && rank == CL - 1;         // owns i = N-2; i = N-1 is its halo
+    const int gw = rank * NW + warp;                     // my warp among the member's NG warps
+    const size_t row = (size_t)b * pb.NP;
+
+    // sync points: S is double-buffered by the parity of its index, F is single
+    const uint32_t mbS0 = smem_u32(smem + L::o_mbar), mbS1 = mbS0 + 8, mbF = mbS0 + 16;
+    // transaction bytes this CTA receives from its peers per sync
+    const uint32_t txS = MULTI ? (uint32_t)((rank > 0 ? 48 : 0) + (rank < CL - 1 ? 48 : 0) + (CL - 1) * NW * 16) : 0u;
+    const uint32_t txF = MULTI ? (uint32_t)((rank > 0 ? 32 : 0) + (rank < CL - 1 ? 32 : 0)) : 0u;
+    if (tid == 0) {
+        mbar_init(mbS0, NW); mbar_init(mbS1, NW); mbar_init(mbF, NW);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+
+    // ---- load: own points to registers, u^n and tables to shared memory
+    double ph[P], pi[P], a[P];
+    double accP[ACC_REG ? P : 1], accQ[ACC_REG ? P : 1], accA[ACC_REG ? P : 1];
+    {
+        const double2 *s0 = reinterpret_cast<const double2 *>(prm.U[0] + row + g0);
+        const double2 *s1 = reinterpret_cast<const double2 *>(prm.U[1] + row + g0);
+        const double2 *s2 = reinterpret_cast<const double2 *>(prm.U[2] + row + g0);
+#pragma unroll
+        for (int p = 0; p < P; p += 2) {
+            double2 v0 = s0[p / 2], v1 = s1[p / 2], v2 = s2[p / 2];
+            ph[p] = v0.x; ph[p + 1] = v0.y; pi[p] = v1.x; pi[p + 1] = v1.y; a[p] = v2.x; a[p + 1] = v2.y;
+        }
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            un[(0 * P + p) * THREADS + tid] = ph[p];
+            un[(1 * P + p) * THREADS + tid] = pi[p];
+            un[(2 * P + p) * THREADS + tid] = a[p];
+            tSC[p * LD + col] = -2.0 * prm.tb.sc[g0 + p];
+            tT[p * THREADS + tid] = prm.tb.T[g0 + p];
+            tC[p * THREADS + tid] = prm.tb.C[g0 + p] * K.d4c;
+            if constexpr (ACC_REG) { accP[p] = ph[p]; accQ[p] = pi[p]; accA[p] = a[p]; }
+            else { accS[(0 * P + p) * THREADS + tid] = ph[p]; accS[(1 * P + p) * THREADS + tid] = pi[p]; accS[(2 * P + p) * THREADS + tid] = a[p]; }
+        }
+        if (lo_edge) tSC[(P - 1) * LD + 0] = -2.0 * prm.tb.sc[g0 - 1];            // odd ghost at x=0
+        if (hi_edge) tSC[0 * LD + THREADS + 1] = -2.0 * prm.tb.sc[g0 + P];        // 0 at x=pi/2
+    }
+    // mbarrier initialisation must be visible to every thread (and peer CTA) that arrives or stores on it
+    if (MULTI) {
+        asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    } else {
+        __syncthreads();
+    }
+
+    // Kept across sync S: f' = -2 f of the own points (fo), thread-local suffix sums s_p (so), the
+    // exclusive warp-level suffix (excl), and the own-point part of the Kreiss-Oliger sums (kP, kQ).
+    double fo[P], so[P], excl, kP[P], kQ[P];
+    int bad = 0;
+
+    // One elected lane per warp arrives; __syncwarp orders the other lanes' shared-memory stores before it.
+    auto warp_arrive = [&](uint32_t mb, uint32_t tx) {
+        __syncwarp();
+        if (lane == 0) {
+            if (MULTI && warp == 0) mbar_arrive_expect_tx(mb, tx);
+            else mbar_arrive(mb);
+        }
+    };
+
+    // f', s of the new state; publish the state edges and the warp total for sync S with index parity jb.
+    auto publish_S = [&](const int jb, const bool with_flag) {
+        const uint32_t mb = jb ? mbS1 : mbS0;
+#pragma unroll
+        for (int p = 0; p < P; ++p) fo[p] = tSC[p * LD + col] * fma(ph[p], ph[p], pi[p] * pi[p]);
+        // top term of the telescoped rule: S_{N-1} = S_N = f_{N-2}/12 (f_N = -f_{N-2}, f_{N-1} = 0)
+        so[P - 1] = fo[P - 1] + (last ? fo[P - 1] * (1.0 / 12.0) : 0.0);
+#pragma unroll
+        for (int p = P - 2; p >= 0; --p) so[p] = so[p + 1] + fo[p];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            xPhi[k * LD + col] = ph[k]; xPi[k * LD + col] = pi[k];
+            xPhi[(RX - 3 + k) * LD + col] = ph[P - 3 + k]; xPi[(RX - 3 + k) * LD + col] = pi[P - 3 + k];
+        }
+        if (lo_edge) {
+            if (rank == 0) {            // x=0: Phi odd, Pi even (R2)
+#pragma unroll
+                for (int k = 1; k <= 3; ++k) { xPhi[(RX - k) * LD] = -ph[k]; xPi[(RX - k) * LD] = pi[k]; }
+            } else if (MULTI) {         // right halo column of the CTA below
+                const uint32_t rmb = map_rank(mb, rank - 1);
+                const uint32_t rP = map_rank(smem_u32(xPhi + THREADS + 1), rank - 1);
+                const uint32_t rQ = map_rank(smem_u32(xPi + THREADS + 1), rank - 1);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    st_async_f64(rP + k * LD * 8, ph[k], rmb); st_async_f64(rQ + k * LD * 8, pi[k], rmb);
+                }
+            }
+        }
+        if (hi_edge) {
+            if (rank == CL - 1) {       // x=pi/2: Phi even, Pi odd, Dirichlet values (R3, eqs 9, 10)
+                xPhi[0 * LD + THREADS + 1] = 0.0;        xPi[0 * LD + THREADS + 1] = 0.0;
+                xPhi[1 * LD + THREADS + 1] = ph[P - 1];  xPi[1 * LD + THREADS + 1] = -pi[P - 1];
+                xPhi[2 * LD + THREADS + 1] = ph[P - 2];  xPi[2 * LD + THREADS + 1] = -pi[P - 2];
+            } else if (MULTI) {         // left halo column of the CTA above
+                const uint32_t rmb = map_rank(mb, rank + 1);
+                const uint32_t rP = map_rank(smem_u32(xPhi), rank + 1);
+                const uint32_t rQ = map_rank(smem_u32(xPi), rank + 1);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    st_async_f64(rP + (RX - 3 + k) * LD * 8, ph[P - 3 + k], rmb);
+                    st_async_f64(rQ + (RX - 3 + k) * LD * 8, pi[P - 3 + k], rmb);
+                }
+            }
+        }
+        // a2, warp level: inclusive suffix over the lanes; the warp total (and collapse flag) goes to every CTA
+        const double incl = warp_suffix_incl(so[0]);
+        excl = incl - so[0];
+        const double wsum = __shfl_sync(FULL, incl, 0);
+        double flag = 0.0;
+        if (with_flag) flag = __any_sync(FULL, bad) ? 1.0 : 0.0;
+        double2 *slot = wt + jb * NG + gw;
+        if (lane == 0) *slot = make_double2(wsum, flag);
+        if (MULTI) {
+            if (lane < CL && lane != rank)
+                st_async_f64x2(map_rank(smem_u32(slot), lane), wsum, flag, map_rank(mb, lane));
+        }
+        warp_arrive(mb, txS);
+    };
+    // Own-point part of Q Phi, Q Pi (R6) of the state in ph, pi; the halo part is added after sync S.
+    auto ko_own = [&]() {
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            double sP = K.kw[0] * ph[p], sQ = K.kw[0] * pi[p];
+#pragma unroll
+            for (int j = 1; j <= 3; ++j) {
+                if (p - j >= 0) { sP = fma(K.kw[j], ph[p - j], sP); sQ = fma(K.kw[j], pi[p - j], sQ); }
+                if (p + j < P)  { sP = fma(K.kw[j], ph[p + j], sP); sQ = fma(K.kw[j], pi[p + j], sQ); }
+            }
+            kP[p] = sP; kQ[p] = sQ;
+        }
+    };
+
+    publish_S(0, false);
+    ko_own();
+    mbar_wait<MULTI>(mbS0, 0);
+
+    long long n_done = 0;
+    int collapsed = 0;
+#pragma unroll 1
+    for (long long n = 0; n < prm.nsteps; ++n) {
+#pragma unroll 1
+        for (int s = 0; s < 4; ++s) {
+            const double a_next = K.a_next[s], b_w = K.b_w[s];
+            // sync S index j = 4n+s: buffer s&1; sync F index 4n+s: parity s&1
+            const double2 *wts = wt + (s & 1) * NG;
+
+            // ---------------------------------------------------------------- phase 1 (after sync S)
+            double hlP[3], hrP[3], hlQ[3], hrQ[3];    // 3 halo points per side of the stage state
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                hlP[k] = xPhi[(RX - 3 + k) * LD + col - 1]; hlQ[k] = xPi[(RX - 3 + k) * LD + col - 1];
+                hrP[k] = xPhi[k * LD + col + 1];            hrQ[k] = xPi[k * LD + col + 1];
+            }
+            const double scm = tSC[(P - 1) * LD + col - 1], scp = tSC[0 * LD + col + 1];
+            // a2, member level: all f' above this thread's points (predicates are warp- / CTA-uniform)
+            double B0 = excl, B1 = 0.0;
+            {
+                const double2 *wl = wts + rank * NW;
+#pragma unroll
+                for (int w = 1; w < NW; ++w) {
+                    if (w > warp) { if (w & 1) B1 += wl[w].x; else B0 += wl[w].x; }
+                }
+                if (MULTI) {
+#pragma unroll
+                    for (int r = 1; r < CL; ++r) {
+                        if (r > rank) {
+#pragma unroll
+                            for (int w = 0; w < NW; ++w) { if (w & 1) B1 += wts[r * NW + w].x; else B0 += wts[r * NW + w].x; }
+                        }
+                    }
+                }
+            }
+            const double B = B0 + B1;
+            // halo part of the Kreiss-Oliger sums
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+#pragma unroll
+                for (int j = 1; j <= 3; ++j) {
+                    if (p - j < 0) { kP[p] = fma(K.kw[j], hlP[3 + p - j], kP[p]); kQ[p] = fma(K.kw[j], hlQ[3 + p - j], kQ[p]); }
+                    if (p + j >= P) { kP[p] = fma(K.kw[j], hrP[p + j - P], kP[p]); kQ[p] = fma(K.kw[j], hrQ[p + j - P], kQ[p]); }
+                }
+            }
+            // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f
+            double nd[P];
+            {
+                const double fm = scm * fma(hlP[2], hlP[2], hlQ[2] * hlQ[2]);     // f'_{-1}
+                const double fp = scp * fma(hrP[0], hrP[0], hrQ[0] * hrQ[0]);     // f'_{P}
+                const double top = last ? fo[P - 1] * (1.0 / 12.0) : 0.0;         // as in publish_S
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const double f_lo = (p == 0) ? fm : fo[p - 1];
+                    const double f_hi = (p == P - 1) ? fp : fo[p + 1];
+                    const double s2 = (p + 2 < P) ? so[p + 2] : ((p + 2 == P) ? top : top - fp);
+                    double loc = K.c25 * f_hi;
+                    loc = fma(K.c12, fo[p], loc);
+                    loc = fma(-K.c1, f_lo, loc);
+                    nd[p] = fma(K.hh, s2 + B, loc);
+                }
+            }
+            double E[P];
+            exp3_near<P>(nd, E);
+            // a3 fluxes
+            double H[P], F[P], kAv[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                const double AE = a[p] * E[p];
+                const double G = AE * ph[p];
+                H[p] = AE * pi[p];
+                F[p] = tT[p * THREADS + tid] * G;
+                if (p == 1) G1 = G;
+                if (p == 2) G2 = G;
+                if (p == P - 1) Gl1 = G;
+                if (p == P - 2) Gl2 = G;
+                kAv[p] = (tSC[p * LD + col] * a[p]) * (G * pi[p]);        // eq (4): -2 sc A G Pi
+            }
+            if (first) kAv[0] = 0.0;                                      // A(0,t)=1, eq (8)
+            // publish flux edges
+            xH[0 * LD + col] = H[0]; xH[1 * LD + col] = H[1]; xH[2 * LD + col] = H[P - 2]; xH[3 * LD + col] = H[P - 1];
+            xF[0 * LD + col] = F[0]; xF[1 * LD + col] = F[1]; xF[2 * LD + col] = F[P - 2]; xF[3 * LD + col] = F[P - 1];
+            if (lo_edge) {
+                if (rank == 0) {       // x=0: H even, F odd
+                    xH[2 * LD] = H[2]; xH[3 * LD] = H[1]; xF[2 * LD] = -F[2]; xF[3 * LD] = -F[1];
+                } else if (MULTI) {
+                    const uint32_t rmb = map_rank(mbF, rank - 1);
+                    const uint32_t rH = map_rank(smem_u32(xH + THREADS + 1), rank - 1);
+                    const uint32_t rF = map_rank(smem_u32(xF + THREADS + 1), rank - 1);
+                    st_async_f64(rH, H[0], rmb); st_async_f64(rH + LD * 8, H[1], rmb);
+                    st_async_f64(rF, F[0], rmb); st_async_f64(rF + LD * 8, F[1], rmb);
+                }
+            }
+            if (hi_edge) {
+                if (rank == CL - 1) {  // x=pi/2: H odd with H=0 there; F even with the limit of R5
+                    xH[0 * LD + THREADS + 1] = 0.0; xH[1 * LD + THREADS + 1] = -H[P - 1];
+                    xF[0 * LD + THREADS + 1] = (16.0 * Gl1 - Gl2) * K.inv12h2;
+                    xF[1 * LD + THREADS + 1] = F[P - 1];
+                } else if (MULTI) {
+                    const uint32_t rmb = map_rank(mbF, rank + 1);
+                    const uint32_t rH = map_rank(smem_u32(xH), rank + 1);
+                    const uint32_t rF = map_rank(smem_u32(xF), rank + 1);
+                    st_async_f64(rH + 2 * LD * 8, H[P - 2], rmb); st_async_f64(rH + 3 * LD * 8, H[P - 1], rmb);
+                    st_async_f64(rF + 2 * LD * 8, F[P - 2], rmb); st_async_f64(rF + 3 * LD * 8, F[P - 1], rmb);
+                }
+            }
+            warp_arrive(mbF, txF);                                        // sync F: arrive
+
+            // ---------------------------------------------------------------- between arrive and wait
+            // a4/a5 for A (eq 4 needs no neighbour).  Invariant at the start of every step: acc == u^n == state.
+            if (s < 3) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int ui = (2 * P + p) * THREADS + tid;
+                    if constexpr (ACC_REG) accA[p] = fma(b_w, kAv[p], accA[p]);
+                    else accS[ui] = fma(b_w, kAv[p], accS[ui]);
+                    a[p] = fma(a_next, kAv[p], un[ui]);
+                }
+            } else {
+                bad = 0;
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int ui = (2 * P + p) * THREADS + tid;
+                    double accn;
+                    if constexpr (ACC_REG) { accn = fma(b_w, kAv[p], accA[p]); accA[p] = accn; }
+                    else { accn = fma(b_w, kAv[p], accS[ui]); accS[ui] = accn; }
+                    a[p] = accn; un[ui] = accn;
+                    if (!(accn >= K.thr)) bad = 1;
+                }
+            }
+            // interior centred differences (own fluxes only)
+            double dH[P], dF[P];
+#pragma unroll
+            for (int p = 2; p < P - 2; ++p) {
+                dH[p] = fma(8.0, H[p + 1] - H[p - 1], H[p - 2] - H[p + 2]);
+                dF[p] = fma(8.0, F[p + 1] - F[p - 1], F[p - 2] - F[p + 2]);
+            }
+            mbar_wait<MULTI>(mbF, (uint32_t)(s & 1));                     // sync F: wait
+
+            // ---------------------------------------------------------------- phase 2
+            {
+                const double Hm2 = xH[2 * LD + col - 1], Hm1 = xH[3 * LD + col - 1];
+                const double Fm2 = xF[2 * LD + col - 1], Fm1 = xF[3 * LD + col - 1];
+                const double Hp0 = xH[0 * LD + col + 1], Hp1 = xH[1 * LD + col + 1];
+                const double Fp0 = xF[0 * LD + col + 1], Fp1 = xF[1 * LD + col + 1];
+                dH[0] = fma(8.0, H[1] - Hm1, Hm2 - H[2]);
+                dF[0] = fma(8.0, F[1] - Fm1, Fm2 - F[2]);
+                dH[1] = fma(8.0, H[2] - H[0], Hm1 - H[3]);
+                dF[1] = fma(8.0, F[2] - F[0], Fm1 - F[3]);
+                dH[P - 2] = fma(8.0, H[P - 1] - H[P - 3], H[P - 4] - Hp0);
+                dF[P - 2] = fma(8.0, F[P - 1] - F[P - 3], F[P - 4] - Fp0);
+                dH[P - 1] = fma(8.0, Hp0 - H[P - 2], H[P - 3] - Hp1);
+                dF[P - 1] = fma(8.0, Fp0 - F[P - 2], F[P - 3] - Fp1);
+            }
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                const double qq = kQ[p];
+                kP[p] = fma(K.d4c, dH[p], kP[p]);
+                kQ[p] = fma(tC[p * THREADS + tid], dF[p], qq);
+                if (p == 0 && first) {           // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
+                    kP[0] = 0.0;
+                    kQ[0] = fma(8.0 * G1 - G2, K.c_org, qq);
+                }
+            }
+            // a5: new stage state first (the scan needs it), accumulators after the shuffle chain started
+            double kPs[P], kQs[P];
+            if (s < 3) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
+                    kPs[p] = kP[p]; kQs[p] = kQ[p];
+                    ph[p] = fma(a_next, kP[p], un[uP]); pi[p] = fma(a_next, kQ[p], un[uQ]);
+                }
+            } else {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
+                    double nP, nQ;
+                    if constexpr (ACC_REG) { nP = fma(b_w, kP[p], accP[p]); nQ = fma(b_w, kQ[p], accQ[p]); accP[p] = nP; accQ[p] = nQ; }
+                    else { nP = fma(b_w, kP[p], accS[uP]); nQ = fma(b_w, kQ[p], accS[uQ]); accS[uP] = nP; accS[uQ] = nQ; }
+                    ph[p] = nP; pi[p] = nQ; un[uP] = nP; un[uQ] = nQ;
+                }
+            }
+            const int jb = (s + 1) & 1;                                   // buffer of the next sync S
+            publish_S(jb, s == 3);                                        // sync S: arrive
+            if (s < 3) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
+                    if constexpr (ACC_REG) { accP[p] = fma(b_w, kPs[p], accP[p]); accQ[p] = fma(b_w, kQs[p], accQ[p]); }
+                    else { accS[uP] = fma(b_w, kPs[p], accS[uP]); accS[uQ] = fma(b_w, kQs[p], accS[uQ]); }
+                }
+            }
+            ko_own();                                                     // for the next stage
+            mbar_wait<MULTI>(jb ? mbS1 : mbS0, (uint32_t)(((s + 1) >> 1) & 1));   // sync S: wait
+            if (s == 3) {
+                // a6: collapse test of PAPER.md:85 on A^{n+1}: every warp of the member published its flag
+                int any = 0;
+                const int2 *fl = reinterpret_cast<const int2 *>(wt + jb * NG);
+#pragma unroll
+                for (int w = 0; w < NG; ++w) any |= fl[2 * w + 1].y;      // high word of the flag (0.0 or 1.0)
+                n_done = n + 1;
+                if (any && (prm.check_last || n + 1 < prm.nsteps)) collapsed = 1;
+            }
+        }
+        if (collapsed) break;                                             // uniform over the cluster
+    }
+
+    // ---- store
+    {
+        double2 *d0 = reinterpret_cast<double2 *>(prm.U[0] + row + g0);
+        double2 *d1 = reinterpret_cast<double2 *>(prm.U[1] + row + g0);
+        double2 *d2 = reinterpret_cast<double2 *>(prm.U[2] + row + g0);
+#pragma unroll
+        for (int p = 0; p < P; p += 2) {
+            d0[p / 2] = make_double2(ph[p], ph[p + 1]);
+            d1[p / 2] = make_double2(pi[p], pi[p + 1]);
+            d2[p / 2] = make_double2(a[p], a[p + 1]);
+        }
+    }
+    if (first) {
+        const long long sd = rec->steps_done + n_done;
+        rec->steps_done = sd;
+        if (collapsed) { rec->collapsed = 1; rec->t_collapse = (double)sd * pb.dt; }
+    }
+    // no CTA may exit while a peer can still store into its shared memory
+    if (MULTI) asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// ------------------------------------------------------------------ configuration table
+#define ADSC_RES3_FN(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_>
+#define ADSC_RES3_CFG_ALL(P_, T_, ACC_)                                                               \
+    { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 8>::bytes, false,       \
+      { ADSC_RES3_FN(P_, T_, ACC_, 1), ADSC_RES3_FN(P_, T_, ACC_, 2), ADSC_RES3_FN(P_, T_, ACC_, 4),    \
+        ADSC_RES3_FN(P_, T_, ACC_, 8) } }
+#define ADSC_RES3_CFG_ONE(P_, T_, ACC_)                                                               \
+    { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 1>::bytes, false,       \
+      { ADSC_RES3_FN(P_, T_, ACC_, 1), nullptr, nullptr, nullptr } }
+
+const ResConfig g_cfgs3[] = {
+    ADSC_RES3_CFG_ALL(8, 256, true),    // SEG 2048, accumulators in registers: N-1 = 2048, 4096, 8192, 16384
+    ADSC_RES3_CFG_ONE(8, 128, false),   // SEG 1024
+    ADSC_RES3_CFG_ONE(4, 128, false),   // SEG 512
+    ADSC_RES3_CFG_ONE(4, 64, false),    // SEG 256
+    ADSC_RES3_CFG_ONE(4, 32, false),    // SEG 128
+};
+const int n_cfgs3 = sizeof(g_cfgs3) / sizeof(g_cfgs3[0]);
+
+}  // namespace adsc
