@@ -172,7 +172,7 @@ __device__ __forceinline__ void st_async_f64x2(uint32_t dst_cluster, double v0, 
 }
 
 template <int P, int THREADS, bool ACC_REG, int CL>
-__global__ void __launch_bounds__(THREADS, 1) k_resident3(const __grid_constant__ ResParams prm)
+__global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resident3(const __grid_constant__ ResParams prm)
 {
     using L = Res3Layout<P, THREADS, ACC_REG, CL>;
     constexpr bool MULTI = CL > 1;
@@ -578,6 +578,8 @@ const ResConfig g_cfgs3[] = {
     ADSC_RES3_CFG_ONE(4, 128, false),   // SEG 512
     ADSC_RES3_CFG_ONE(4, 64, false),    // SEG 256
     ADSC_RES3_CFG_ONE(4, 32, false),    // SEG 128
+    ADSC_RES3_CFG_ALL(8, 128, true),    // SEG 1024, two CTAs per SM (tuning)
+    ADSC_RES3_CFG_ALL(4, 512, true),    // SEG 2048, 16 warps (tuning)
 };
 const int n_cfgs3 = sizeof(g_cfgs3) / sizeof(g_cfgs3[0]);
 
