@@ -178,6 +178,14 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
     constexpr bool MULTI = CL > 1;
     constexpr int LD = L::LD, NW = L::NW, NG = L::NG, SEG = L::SEG, RX = L::RX;
     constexpr unsigned FULL = 0xffffffffu;
+#ifndef ADSC_R3_EARLY
+#define ADSC_R3_EARLY 0
+#endif
+#ifndef ADSC_R3_NFILL
+#define ADSC_R3_NFILL 3
+#endif
+    constexpr bool EARLY = ADSC_R3_EARLY && (P >= 6);                   // interior right-hand sides before the sync-F wait
+    constexpr int NFILL = (P < ADSC_R3_NFILL) ? P : ADSC_R3_NFILL;      // Kreiss-Oliger points computed inside the shuffle chain
     extern __shared__ __align__(16) double smem[];
     double *xPhi = smem + L::o_xPhi, *xPi = smem + L::o_xPi, *xH = smem + L::o_xH, *xF = smem + L::o_xF;
     double *tSC = smem + L::o_tSC, *tT = smem + L::o_tT, *tC = smem + L::o_tC;
@@ -256,6 +264,16 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
         }
     };
 
+    // Own-point part of Q Phi, Q Pi (R6) of the state in ph, pi at point p; the halo part is added after sync S.
+    auto ko_pt = [&](const int p) {
+        double sP = K.kw[0] * ph[p], sQ = K.kw[0] * pi[p];
+#pragma unroll
+        for (int j = 1; j <= 3; ++j) {
+            if (p - j >= 0) { sP = fma(K.kw[j], ph[p - j], sP); sQ = fma(K.kw[j], pi[p - j], sQ); }
+            if (p + j < P)  { sP = fma(K.kw[j], ph[p + j], sP); sQ = fma(K.kw[j], pi[p + j], sQ); }
+        }
+        kP[p] = sP; kQ[p] = sQ;
+    };
     // f', s of the new state; publish the state edges and the warp total for sync S with index parity jb.
     auto publish_S = [&](const int jb, const bool with_flag) {
         const uint32_t mb = jb ? mbS1 : mbS0;
@@ -300,8 +318,16 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 }
             }
         }
-        // a2, warp level: inclusive suffix over the lanes; the warp total (and collapse flag) goes to every CTA
-        const double incl = warp_suffix_incl(so[0]);
+        // a2, warp level: inclusive suffix over the lanes; the warp total (and collapse flag) goes to every CTA.
+        // The shuffle chain (5 dependent steps) is pure latency, so the own-point Kreiss-Oliger sums of the
+        // first NFILL points are written between its steps: one basic block, ptxas interleaves them.
+        double incl = so[0];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const double o = __shfl_down_sync(FULL, incl, 1 << k);
+            if (k < NFILL) ko_pt(k);
+            if (lane + (1 << k) < 32) incl += o;
+        }
         excl = incl - so[0];
         const double wsum = __shfl_sync(FULL, incl, 0);
         double flag = 0.0;
@@ -314,22 +340,14 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
         }
         warp_arrive(mb, txS);
     };
-    // Own-point part of Q Phi, Q Pi (R6) of the state in ph, pi; the halo part is added after sync S.
-    auto ko_own = [&]() {
+    // Own-point part of Q Phi, Q Pi (R6) for points [NFILL, P); publish_S did the first NFILL.
+    auto ko_rest = [&]() {
 #pragma unroll
-        for (int p = 0; p < P; ++p) {
-            double sP = K.kw[0] * ph[p], sQ = K.kw[0] * pi[p];
-#pragma unroll
-            for (int j = 1; j <= 3; ++j) {
-                if (p - j >= 0) { sP = fma(K.kw[j], ph[p - j], sP); sQ = fma(K.kw[j], pi[p - j], sQ); }
-                if (p + j < P)  { sP = fma(K.kw[j], ph[p + j], sP); sQ = fma(K.kw[j], pi[p + j], sQ); }
-            }
-            kP[p] = sP; kQ[p] = sQ;
-        }
+        for (int p = NFILL; p < P; ++p) ko_pt(p);
     };
 
     publish_S(0, false);
-    ko_own();
+    ko_rest();
     mbar_wait<MULTI>(mbS0, 0);
 
     long long n_done = 0;
@@ -463,13 +481,48 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                     if (!(accn >= K.thr)) bad = 1;
                 }
             }
-            // interior centred differences (own fluxes only)
-            double dH[P], dF[P];
+            // interior points p in [2, P-2) need own fluxes only: their differences, right-hand sides and
+            // RK combine are done before the wait, in the shadow of the slowest warp's arrival
+            double dH[P], dF[P], kPs[P], kQs[P];
+            // a4 + a5 for points [p0, p1): new stage state (s < 3; the accumulator update is deferred past
+            // the scan) or the new time level (s = 3)
+            auto rhs_combine = [&](const int p0, const int p1) {
+#pragma unroll
+                for (int p = p0; p < p1; ++p) {
+                    const double qq = kQ[p];
+                    kP[p] = fma(K.d4c, dH[p], kP[p]);
+                    kQ[p] = fma(tC[p * THREADS + tid], dF[p], qq);
+                    if (p == 0 && first) {       // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
+                        kP[0] = 0.0;
+                        kQ[0] = fma(8.0 * G1 - G2, K.c_org, qq);
+                    }
+                }
+                if (s < 3) {
+#pragma unroll
+                    for (int p = p0; p < p1; ++p) {
+                        const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
+                        kPs[p] = kP[p]; kQs[p] = kQ[p];
+                        ph[p] = fma(a_next, kP[p], un[uP]); pi[p] = fma(a_next, kQ[p], un[uQ]);
+                    }
+                } else {
+#pragma unroll
+                    for (int p = p0; p < p1; ++p) {
+                        const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
+                        double nP, nQ;
+                        if constexpr (ACC_REG) { nP = fma(b_w, kP[p], accP[p]); nQ = fma(b_w, kQ[p], accQ[p]); accP[p] = nP; accQ[p] = nQ; }
+                        else { nP = fma(b_w, kP[p], accS[uP]); nQ = fma(b_w, kQ[p], accS[uQ]); accS[uP] = nP; accS[uQ] = nQ; }
+                        ph[p] = nP; pi[p] = nQ; un[uP] = nP; un[uQ] = nQ;
+                    }
+                }
+            };
 #pragma unroll
             for (int p = 2; p < P - 2; ++p) {
                 dH[p] = fma(8.0, H[p + 1] - H[p - 1], H[p - 2] - H[p + 2]);
                 dF[p] = fma(8.0, F[p + 1] - F[p - 1], F[p - 2] - F[p + 2]);
             }
+            // edge operands are taken before the interior state is overwritten (ph, pi are not flux inputs
+            // any more at this point: H, F, G1, G2 hold everything phase 2 needs)
+            if (EARLY) rhs_combine(2, P - 2);
             mbar_wait<MULTI>(mbF, (uint32_t)(s & 1));                     // sync F: wait
 
             // ---------------------------------------------------------------- phase 2
@@ -487,35 +540,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 dH[P - 1] = fma(8.0, Hp0 - H[P - 2], H[P - 3] - Hp1);
                 dF[P - 1] = fma(8.0, Fp0 - F[P - 2], F[P - 3] - Fp1);
             }
-#pragma unroll
-            for (int p = 0; p < P; ++p) {
-                const double qq = kQ[p];
-                kP[p] = fma(K.d4c, dH[p], kP[p]);
-                kQ[p] = fma(tC[p * THREADS + tid], dF[p], qq);
-                if (p == 0 && first) {           // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
-                    kP[0] = 0.0;
-                    kQ[0] = fma(8.0 * G1 - G2, K.c_org, qq);
-                }
-            }
-            // a5: new stage state first (the scan needs it), accumulators after the shuffle chain started
-            double kPs[P], kQs[P];
-            if (s < 3) {
-#pragma unroll
-                for (int p = 0; p < P; ++p) {
-                    const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
-                    kPs[p] = kP[p]; kQs[p] = kQ[p];
-                    ph[p] = fma(a_next, kP[p], un[uP]); pi[p] = fma(a_next, kQ[p], un[uQ]);
-                }
-            } else {
-#pragma unroll
-                for (int p = 0; p < P; ++p) {
-                    const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
-                    double nP, nQ;
-                    if constexpr (ACC_REG) { nP = fma(b_w, kP[p], accP[p]); nQ = fma(b_w, kQ[p], accQ[p]); accP[p] = nP; accQ[p] = nQ; }
-                    else { nP = fma(b_w, kP[p], accS[uP]); nQ = fma(b_w, kQ[p], accS[uQ]); accS[uP] = nP; accS[uQ] = nQ; }
-                    ph[p] = nP; pi[p] = nQ; un[uP] = nP; un[uQ] = nQ;
-                }
-            }
+            if (EARLY) { rhs_combine(0, 2); rhs_combine(P - 2, P); }
+            else rhs_combine(0, P);
             const int jb = (s + 1) & 1;                                   // buffer of the next sync S
             publish_S(jb, s == 3);                                        // sync S: arrive
             if (s < 3) {
@@ -526,7 +552,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                     else { accS[uP] = fma(b_w, kPs[p], accS[uP]); accS[uQ] = fma(b_w, kQs[p], accS[uQ]); }
                 }
             }
-            ko_own();                                                     // for the next stage
+            ko_rest();                                                    // for the next stage
             mbar_wait<MULTI>(jb ? mbS1 : mbS0, (uint32_t)(((s + 1) >> 1) & 1));   // sync S: wait
             if (s == 3) {
                 // a6: collapse test of PAPER.md:85 on A^{n+1}: every warp of the member published its flag
