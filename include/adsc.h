@@ -47,10 +47,15 @@ extern "C" {
 #define ADSC_OPT_A_RESOLVE_PERIOD   2  /* K_A: every K_A steps A is replaced by the
                                           integral of eq (5) ("periodically integrating
                                           A").  Default 0 = never.          */
-#define ADSC_OPT_PATH               3  /* 0 auto (default), 1 force the streaming
-                                          (global-memory) kernels, 2 force the resident
-                                          (shared-memory/register) kernel; EINVAL if the
-                                          forced path cannot hold N.                    */
+#define ADSC_OPT_PATH               3  /* 0 auto (default: resident if a member fits on
+                                          chip, else streaming); 1 force the streaming path
+                                          (persistent kernel, stage state in shared memory,
+                                          u^n and accumulator in global memory; falls back
+                                          to 3 at adsc_bind if the member's CTAs cannot all
+                                          be co-resident); 2 force the resident
+                                          (shared-memory/register) kernel, EINVAL if it
+                                          cannot hold N; 3 force the generic streaming
+                                          kernels (one launch per phase, any N).        */
 #define ADSC_OPT_STEPS_PER_LAUNCH   4  /* resident path: RK4 steps per kernel launch
                                           (default 0 = all steps of a call in one launch) */
 
@@ -134,8 +139,9 @@ int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A
 /* Number of kernels this handle has launched since adsc_bind (for gpu_launches). */
 long long adsc_launch_count(adsc_handle h);
 
-/* Which kernel family adsc_step uses for this handle: 1 streaming, 2 resident;
- * *cluster (may be NULL) receives the CTAs per member of the resident path. */
+/* Which kernel family adsc_step uses for this handle (final after adsc_bind): 1 persistent
+ * streaming, 2 resident, 3 generic streaming; *cluster (may be NULL) receives the CTAs
+ * per member (cluster size of the resident path, chunks of the persistent streaming path). */
 int adsc_path(adsc_handle h, int *cluster);
 
 /* Text of the last error on this handle (or of the last failed adsc_create if

@@ -21,7 +21,7 @@ static void compute_layout(adsc_ctx *c)
     const size_t ext = align_up((size_t)c->pb.B * c->pb.N * sizeof(double), 256);
     L.ntiles = (c->pb.N + GEN_TILE - 1) / GEN_TILE;
     const size_t tiles = align_up((size_t)c->pb.B * L.ntiles * sizeof(double), 256);
-    const bool stream = (c->path == 1);
+    const bool stream = (c->path != 2);
     size_t off = 0;
     for (int v = 0; v < 3; ++v) { L.off_U[v] = off; off += field; }
     for (int v = 0; v < 3; ++v) { L.off_Ua[v] = off; off += stream ? field : 0; }
@@ -34,13 +34,15 @@ static void compute_layout(adsc_ctx *c)
     for (int k = 0; k < 2; ++k) { L.off_stage[k] = off; off += ext; }
     L.off_tab = off; off += align_up((size_t)5 * (c->pb.NP + 2 * HAL) * sizeof(double), 256);
     L.off_rec = off; off += align_up((size_t)c->pb.B * sizeof(MemberRec), 256);
+    L.off_mbox = off; off += align_up((size_t)SP_MAX_CTAS * 2 * 24 * sizeof(double), 256);
+    L.off_cnt = off; off += align_up((size_t)SP_MAX_CTAS * sizeof(unsigned long long), 256);
     L.total = off;
 }
 
 static void resolve_path(adsc_ctx *c)
 {
     const bool can_res = resident_select(c);
-    if (c->path_opt == 1) c->path = 1;
+    if (c->path_opt == 1 || c->path_opt == 3) c->path = c->path_opt;
     else if (c->path_opt == 2) c->path = can_res ? 2 : 0;
     else c->path = can_res ? 2 : 1;
     if (c->path != 2) c->cluster = 1;
@@ -85,6 +87,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
     c->cluster = 1; c->res_cfg = -1; c->res_force = -1;
+    c->sp_ok = false; c->sp_G = 0; c->sp_groups = 0; c->sp_Lc = 0;
     resolve_path(c);
     return c;
 }
@@ -115,7 +118,7 @@ int adsc_set_option(adsc_handle h, int key, double value)
         h->K_A = (int)value;
         return ADSC_OK;
     case ADSC_OPT_PATH: {
-        if (!(value == 0.0 || value == 1.0 || value == 2.0)) return fail(h, ADSC_EINVAL, "path must be 0, 1 or 2");
+        if (!(value == 0.0 || value == 1.0 || value == 2.0 || value == 3.0)) return fail(h, ADSC_EINVAL, "path must be 0, 1, 2 or 3");
         if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_PATH before adsc_bind");
         const int old = h->path_opt;
         h->path_opt = (int)value;
@@ -178,6 +181,10 @@ int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream)
     h->ws.stage[1] = (double *)(base + L.off_stage[1]);
     h->ws.tab = (double *)(base + L.off_tab);
     h->ws.rec = (MemberRec *)(base + L.off_rec);
+    h->ws.sp_mbox = (double *)(base + L.off_mbox);
+    h->ws.sp_counter = (unsigned long long *)(base + L.off_cnt);
+    // the persistent streaming kernel needs every CTA of a member co-resident; otherwise one kernel per phase
+    if (h->path == 1 && !stream_persist_select(h)) h->path = 3;
     const size_t NT = (size_t)h->pb.NP + 2 * HAL;
     h->tb.sc = h->ws.tab + 0 * NT + HAL;
     h->tb.T = h->ws.tab + 1 * NT + HAL;
@@ -238,14 +245,15 @@ int adsc_step(adsc_handle h, long long nsteps)
     if (!h->bound || !h->have_state) return fail(h, ADSC_ESTATE, "adsc_bind and adsc_set_initial first");
     if (nsteps < 0) return fail(h, ADSC_EINVAL, "nsteps must be >= 0");
     const int K = h->K_A;
-    if (h->path == 2) {
+    if (h->path == 2 || h->path == 1) {
         long long left = nsteps;
         while (left > 0) {
             long long n = left;
             if (K > 0) { const long long to_b = K - (h->global_step % K); if (n > to_b) n = to_b; }
             if (h->steps_per_launch > 0 && n > h->steps_per_launch) n = h->steps_per_launch;
             const bool hit = K > 0 && ((h->global_step + n) % K == 0);
-            ADSC_CUDA(launch_resident(h, n, hit ? 0 : 1), "resident kernel");
+            if (h->path == 2) ADSC_CUDA(launch_resident(h, n, hit ? 0 : 1), "resident kernel");
+            else ADSC_CUDA(launch_stream_persist(h, n, hit ? 0 : 1), "persistent streaming kernel");
             if (hit) {
                 ADSC_CUDA(launch_solve(h, SOLVE_WRITE_A | SOLVE_ACTIVE_ONLY), "A re-solve");
                 ADSC_CUDA(launch_finalize(h, 0), "finalize");
@@ -328,7 +336,7 @@ long long adsc_launch_count(adsc_handle h) { return h ? h->launches : 0; }
 int adsc_path(adsc_handle h, int *cluster)
 {
     if (!h) return ADSC_EINVAL;
-    if (cluster) *cluster = h->cluster;
+    if (cluster) *cluster = (h->path == 1 && h->sp_ok) ? h->sp_G : h->cluster;
     return h->path;
 }
 

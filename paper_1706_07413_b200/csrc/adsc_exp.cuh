@@ -1,0 +1,76 @@
+// adsc_exp.cuh — branch-free fp64 exponential used by the stage kernels (resident and persistent
+// streaming): e^{-delta} of eqs (2), (3) is the only transcendental on the hot path.
+#pragma once
+
+namespace adsc {
+
+// exp coefficients (read as constant-bank operands)
+static __constant__ double c_exp[18] = {
+    1.4426950408889634074,            // 0  log2 e
+    6755399441055744.0,               // 1  1.5 * 2^52 (round-to-nearest-integer shift)
+    -6.93147180369123816490e-01,      // 2  -ln2 (high part)
+    -1.90821492927058770002e-10,      // 3  -ln2 (low part)
+    1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0, 1.0 / 40320.0,   // 4..10: 1/k!, k=2..8
+    1.0 / 362880.0, 1.0 / 3628800.0, 1.0 / 39916800.0, 1.0 / 479001600.0, 1.0 / 6227020800.0,  // 11..15: k=9..13
+    -708.0, 709.0                     // 16, 17 clamps
+};
+
+// Branch-free e^x (x clamped to [-708, 709]; NaN propagates; e^0 = 1 exactly): k = rint(x log2 e),
+// r = x - k ln 2 in two pieces, Taylor polynomial of degree 13 split in two halves to shorten the
+// dependency chain (|r| <= 0.347: truncation r^14/14! < 5e-18), scaled by 2^k through the exponent field.
+__device__ __forceinline__ double exp3_ref(double x)
+{
+    x = (x < c_exp[16]) ? c_exp[16] : x;
+    x = (x > c_exp[17]) ? c_exp[17] : x;
+    const double t = fma(x, c_exp[0], c_exp[1]);
+    const int k = __double2loint(t);
+    const double kf = t - c_exp[1];
+    double r = fma(kf, c_exp[2], x);
+    r = fma(kf, c_exp[3], r);
+    double lo = fma(r, c_exp[8], c_exp[7]);
+    double hi = fma(r, c_exp[15], c_exp[14]);
+    const double r2 = r * r;
+    lo = fma(r, lo, c_exp[6]);        hi = fma(r, hi, c_exp[13]);
+    const double r3 = r2 * r, r4 = r2 * r2;
+    lo = fma(r, lo, c_exp[5]);        hi = fma(r, hi, c_exp[12]);
+    const double r7 = r4 * r3;
+    lo = fma(r, lo, c_exp[4]);        hi = fma(r, hi, c_exp[11]);
+    lo = fma(r, lo, 1.0);             hi = fma(r, hi, c_exp[10]);
+    lo = fma(r, lo, 1.0);             hi = fma(r, hi, c_exp[9]);
+    const double e = fma(r7, hi, lo);
+    return e * __hiloint2double((k + 1023) << 20, 0);
+}
+
+// e^{x_p} for P values that lie close together: one exp at the reference x_{P-1}, the rest
+// relative to it.  exp(z) = 1 + z t(z), t = sum_{k<=5} z^k/(k+1)!; for |z| <= 2^-6 the truncation
+// is z^7/5040 < 5e-17 relative.  x = 0 gives exactly 1 (pure AdS stays bit-exact).
+template <int P>
+__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P])
+{
+    const double xr = x[P - 1];
+    double z[P];
+    int big = 0;
+#pragma unroll
+    for (int p = 0; p < P - 1; ++p) {
+        z[p] = x[p] - xr;
+        big |= ((__double2hiint(z[p]) & 0x7fffffff) > 0x3f900000) ? 1 : 0;    // |z| > 2^-6 (or NaN)
+    }
+    const double Er = exp3_ref(xr);
+    E[P - 1] = Er;
+    if (!big) {
+#pragma unroll
+        for (int p = 0; p < P - 1; ++p) {
+            double t = fma(z[p], c_exp[8], c_exp[7]);
+            t = fma(z[p], t, c_exp[6]);
+            t = fma(z[p], t, c_exp[5]);
+            t = fma(z[p], t, c_exp[4]);
+            t = fma(z[p], t, 1.0);
+            E[p] = fma(Er * z[p], t, Er);
+        }
+    } else {
+#pragma unroll
+        for (int p = 0; p < P - 1; ++p) E[p] = exp3_ref(x[p]);
+    }
+}
+
+}  // namespace adsc

@@ -13,6 +13,7 @@ namespace adsc {
 constexpr int HAL = 4;            // table halo on each side (3 used by the widest stencil)
 constexpr int GEN_TILE = 1024;    // points per CTA tile of the streaming kernels
 constexpr int GEN_THREADS = 256;  // 4 points per thread
+constexpr int SP_MAX_CTAS = 1024; // persistent streaming kernel: mailbox / barrier slots in the workspace
 
 // Per-member record kept on the device (copied to the host by adsc_diagnostics).
 struct MemberRec {
@@ -53,13 +54,15 @@ struct Workspace {
     double *tot;         // streaming: [B][ntiles] tile totals
     double *carry;       // streaming: [B][ntiles] exclusive suffix of tot
     double *stage[2];    // host staging [B][N]
+    double *sp_mbox;     // persistent streaming: [SP_MAX_CTAS][2][24] chunk mailboxes
+    unsigned long long *sp_counter;   // persistent streaming: [SP_MAX_CTAS] group barrier counters
     double *tab;         // 5 tables
     MemberRec *rec;      // [B]
 };
 
 struct Layout {
     size_t off_U[3], off_Ua[3], off_Ub[3], off_ACC[3], off_dl, off_Ac, off_tot, off_carry,
-        off_stage[2], off_tab, off_rec, total;
+        off_stage[2], off_tab, off_rec, off_mbox, off_cnt, total;
     int ntiles;
 };
 
@@ -71,7 +74,7 @@ struct adsc_ctx {
     int K_A;                 // A re-solve period (0 = never)
     int path_opt;            // ADSC_OPT_PATH
     long long steps_per_launch;
-    int path;                // resolved: 1 streaming, 2 resident
+    int path;                // resolved: 1 streaming (persistent), 2 resident, 3 streaming (one kernel per phase)
     int cluster;             // CTAs per member (resident)
     int res_cfg;             // index into the resident configuration table
     int res_force;           // ADSC_OPT_RESIDENT_VARIANT: -1 auto, else the only table entry tried
@@ -85,6 +88,8 @@ struct adsc_ctx {
     long long global_step;   // steps since set_initial (lock-step over active members)
     int dev_sms;
     int dev_smem_optin;
+    bool sp_ok;              // persistent streaming kernel usable (decided at adsc_bind)
+    int sp_G, sp_groups, sp_Lc;   // chunks per member, concurrent members, points per chunk
     std::string err;
 };
 
@@ -98,7 +103,9 @@ cudaError_t launch_unpack(adsc_ctx *c, const double *src_internal, double *dst);
 enum { SOLVE_WRITE_A = 1, SOLVE_DIAG = 2, SOLVE_ACTIVE_ONLY = 4 };
 cudaError_t launch_solve(adsc_ctx *c, int mode);
 cudaError_t launch_finalize(adsc_ctx *c, int inc_steps);
-cudaError_t launch_stream_step(adsc_ctx *c);                 // one RK4 step, streaming path
+cudaError_t launch_stream_step(adsc_ctx *c);                 // one RK4 step, generic streaming kernels
+bool stream_persist_select(adsc_ctx *c);                     // fills c->sp_* (needs c->dev_sms)
+cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last);   // persistent streaming kernel
 cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last);  // resident path
 bool resident_select(adsc_ctx *c);                           // fills c->cluster, c->res_cfg
 const char *resident_cfg_name(int cfg);

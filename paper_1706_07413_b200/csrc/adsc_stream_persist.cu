@@ -1,0 +1,538 @@
+// adsc_stream_persist.cu — persistent streaming kernel: a member too long for one cluster
+// (BASELINE.json configs[3], N = 2^20+1) is cut into G contiguous chunks, one per CTA, one CTA per
+// SM, all co-resident (cooperative launch).  A CTA keeps the STAGE state (Phi*, Pi*, A*) of its
+// chunk in shared memory across all RK stages and steps; u^n and the RK accumulator stream through
+// global memory (L2-resident at this size: 6 arrays x 8.4 MB), 216 B per point per RK4 step.
+//
+// Per RK stage (equations PAPER.md:43-53 eqs (2)-(6); boundary conditions PAPER.md:59-75):
+//   publish   chunk total of f' = -2 sin x cos x (Phi^2 + Pi^2), collapse flag, 3-point state edges
+//   barrier   one grid-wide barrier over the G CTAs of the member (the delta integration of eq (6)
+//             is what the paper calls "order dependent": here it is a three-level
+//             suffix scan, thread / CTA tile / chunk totals)
+//   tiles     walking the chunk from high x to low x (the direction of the suffix scan, R8), per tile
+//             of 1024 points: f', tile scan, delta by the telescoped rule,
+//             E = e^{-delta}, fluxes G, H, F, D4 and Kreiss-Oliger stencils, RK combine, in-place
+//             write of the new stage state, running sum of the NEW state's f' for the next stage.
+// The discrete algorithm is DESIGN.md section 1; nothing here is shared with oracle/.
+#include "adsc_internal.cuh"
+#include "adsc_exp.cuh"
+
+namespace adsc {
+
+constexpr int SP_THREADS = 256;
+constexpr int SP_PPT = 4;                          // contiguous points per thread
+constexpr int SP_TILE = SP_THREADS * SP_PPT;       // 1024
+constexpr int SP_TILES = 7;                        // tiles per chunk
+constexpr int SP_CAP = SP_TILE * SP_TILES;         // 7168 points per CTA
+constexpr int SP_HAL = 4;                          // lower halo slots of the chunk arrays (3 used)
+constexpr int SP_MBOX = 24;                        // doubles per chunk mailbox
+
+// Shared-memory index map: thread t touches 4t+q, a stride of 4 doubles; one padding double per 16
+// makes those accesses conflict-free (16 consecutive lanes fall into 16 distinct 8-byte banks).
+__host__ __device__ constexpr int sp_pad(int j) { return j + (j >> 4); }
+
+struct SPLayout {
+    static constexpr int field = sp_pad(SP_CAP + SP_HAL + 4) + 1;   // one chunk array with lower halo
+    static constexpr int flux = sp_pad(SP_TILE + 4) + 1;            // tile + 2 halo points per side
+    static constexpr int o_S = 0;                                   // [3][field]
+    static constexpr int o_H = o_S + 3 * field;
+    static constexpr int o_F = o_H + flux;
+    static constexpr int o_up = o_F + flux;                         // upP[3], upQ[3], upA[2]
+    static constexpr int o_sw = o_up + 8;                           // scan scratch [40]
+    static constexpr int o_gE = o_sw + 40;                          // G_1, G_2, G_{N-2}, G_{N-3}
+    static constexpr int o_misc = o_gE + 4;                         // carry, top, flags ... [8]
+    static constexpr int n_doubles = o_misc + 8;
+    static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
+};
+
+struct SPConsts {
+    double d4c, kw[4], hh, c25, c12, c1, inv12h2, c_org, a_next[4], b_w[4], thr;
+};
+
+struct SPParams {
+    Problem pb;
+    Tables tb;
+    double *U[3];
+    double *ACC[3];
+    MemberRec *rec;
+    double *mbox;                    // [groups][2][G][SP_MBOX]
+    unsigned long long *counter;     // [groups], zeroed before the launch
+    long long nsteps;
+    int check_last;
+    int G, groups, Lc;               // chunks per member, concurrent members, points per chunk
+    SPConsts k;
+};
+
+// ---- grid barrier over the G CTAs of one member (all co-resident: cooperative launch)
+__device__ __forceinline__ void group_barrier(unsigned long long *cnt, unsigned long long target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(cnt, 1ULL);
+        unsigned long long v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(cnt) : "memory");
+        } while (v < target);
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ double ld_cg(const double *p)
+{
+    double v;
+    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Sum over the CTA (result valid in every thread).  sw: 40 doubles.
+__device__ __forceinline__ double block_sum(double v, double *sw)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    __syncthreads();
+    if (lane == 0) sw[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < SP_THREADS / 32; ++w) t += sw[w];
+    return t;
+}
+
+// Exclusive suffix over the threads of the CTA: sum of S over threads above this one; total in `total`.
+__device__ __forceinline__ double block_suffix_excl_sp(double S, double *sw, double &total)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double incl = warp_suffix_incl(S);
+    __syncthreads();
+    if (lane == 0) sw[warp] = incl;
+    __syncthreads();
+    double above = 0.0, t = 0.0;
+#pragma unroll
+    for (int w = 0; w < SP_THREADS / 32; ++w) {
+        const double x = sw[w];
+        t += x;
+        if (w > warp) above += x;
+    }
+    total = t;
+    return incl - S + above;
+}
+
+__global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_constant__ SPParams prm)
+{
+    using L = SPLayout;
+    extern __shared__ __align__(16) double smem[];
+    double *S = smem + L::o_S, *sH = smem + L::o_H, *sF = smem + L::o_F, *up = smem + L::o_up;
+    double *sw = smem + L::o_sw, *gE = smem + L::o_gE, *misc = smem + L::o_misc;
+    auto Sv = [&](int v, int l) -> double & { return S[v * L::field + sp_pad(l + SP_HAL)]; };
+
+    const Problem &pb = prm.pb;
+    const SPConsts &K = prm.k;
+    const int N = pb.N, G = prm.G, tid = threadIdx.x;
+    const int gi = blockIdx.x / G, c = blockIdx.x - gi * G;
+    if (gi >= prm.groups) return;
+    const int ci0 = c * prm.Lc;                         // first grid index of the chunk
+    const int cn = min(prm.Lc, N - ci0);                // points in the chunk (>= 8 by construction)
+    const int ntile = (cn + SP_TILE - 1) / SP_TILE;
+    const bool owns_top = (ci0 <= N - 2) && (N - 2 < ci0 + cn);     // chunk holding i = N-2
+    unsigned long long *cnt = prm.counter + gi;
+    double *mb = prm.mbox + (size_t)gi * 2 * G * SP_MBOX;
+    unsigned long long epoch = 0;
+    const double *__restrict__ tSC = prm.tb.sc;
+    const double *__restrict__ tT = prm.tb.T;
+    const double *__restrict__ tC = prm.tb.C;
+
+    // value at local index l of field v, l in [tile start - 3, tend + 3): above the tile end the OLD
+    // values live in `up` (the tile above has already been overwritten with the new stage state)
+    auto ldv = [&](int v, int l, int tend) -> double {
+        if (l < tend) return Sv(v, l);
+        const int k = l - tend;
+        if (v == 2) return (k < 2) ? up[6 + k] : 0.0;
+        return (k < 3) ? up[3 * v + k] : 0.0;
+    };
+
+    for (int b = gi; b < pb.B; b += prm.groups) {
+        MemberRec *rec = prm.rec + b;
+        if (rec->collapsed || prm.nsteps <= 0) continue;             // uniform over the group
+        const size_t row = (size_t)b * pb.NP;
+
+        // ---- load the chunk; f' total of the initial state
+        double facc = 0.0;
+        for (int l = tid; l < cn; l += SP_THREADS) {
+            const int i = ci0 + l;
+            const double p = prm.U[0][row + i], q = prm.U[1][row + i];
+            Sv(0, l) = p; Sv(1, l) = q; Sv(2, l) = prm.U[2][row + i];
+            if (i <= N - 2) {
+                const double f = (-2.0 * tSC[i]) * fma(p, p, q * q);
+                facc += f;
+                if (i == N - 2) misc[1] = f * (1.0 / 12.0);          // top term of the telescoped rule
+            }
+        }
+        int bad = 0, collapsed = 0;
+        long long n = 0;
+        unsigned stage_ctr = 0;
+
+        for (;;) {
+            for (int s = 0; s < 4; ++s, ++stage_ctr) {
+                const int par = (int)(stage_ctr & 1u);
+                double *mine = mb + ((size_t)par * G + c) * SP_MBOX;
+                // ---- publish: chunk total (+ top), collapse flag, state edges
+                double tot = block_sum(facc, sw);
+                if (owns_top) tot += misc[1];
+                if (tid == 0) { mine[0] = tot; mine[1] = bad ? 1.0 : 0.0; }
+                if (tid < 3) {
+                    mine[2 + tid] = Sv(0, tid);          mine[5 + tid] = Sv(1, tid);
+                    mine[10 + tid] = Sv(0, cn - 3 + tid); mine[13 + tid] = Sv(1, cn - 3 + tid);
+                }
+                if (tid < 2) { mine[8 + tid] = Sv(2, tid); mine[16 + tid] = Sv(2, cn - 2 + tid); }
+                group_barrier(cnt, (++epoch) * (unsigned long long)G);
+
+                // ---- gather: totals of the chunks above, flags, neighbour edges / parity ghosts
+                const double *all = mb + (size_t)par * G * SP_MBOX;
+                if (tid < 32) {
+                    double cs = 0.0, fl = 0.0;
+                    for (int cc = tid; cc < G; cc += 32) {
+                        const double t = ld_cg(all + (size_t)cc * SP_MBOX), f = ld_cg(all + (size_t)cc * SP_MBOX + 1);
+                        if (cc > c) cs += t;
+                        fl += f;
+                    }
+#pragma unroll
+                    for (int d = 16; d >= 1; d >>= 1) {
+                        cs += __shfl_xor_sync(0xffffffffu, cs, d);
+                        fl += __shfl_xor_sync(0xffffffffu, fl, d);
+                    }
+                    if (tid == 0) { misc[0] = cs + (owns_top ? misc[1] : 0.0); misc[2] = fl; }
+                } else if (tid < 35) {
+                    const int k = tid - 32;                              // 0..2
+                    if (c > 0) {
+                        const double *lo = all + (size_t)(c - 1) * SP_MBOX;
+                        Sv(0, -3 + k) = ld_cg(lo + 10 + k); Sv(1, -3 + k) = ld_cg(lo + 13 + k);
+                        if (k < 2) Sv(2, -2 + k) = ld_cg(lo + 16 + k);
+                    } else {                                             // x = 0: Phi odd, Pi and A even (R2)
+                        Sv(0, -1 - k) = -Sv(0, 1 + k); Sv(1, -1 - k) = Sv(1, 1 + k); Sv(2, -1 - k) = Sv(2, 1 + k);
+                    }
+                    if (c < G - 1) {
+                        const double *hi = all + (size_t)(c + 1) * SP_MBOX;
+                        up[k] = ld_cg(hi + 2 + k); up[3 + k] = ld_cg(hi + 5 + k);
+                        if (k < 2) up[6 + k] = ld_cg(hi + 8 + k);
+                    } else {                                             // x = pi/2: Phi even, Pi odd (R3)
+                        const int lN = N - 1 - ci0;
+                        up[k] = Sv(0, lN - 1 - k); up[3 + k] = -Sv(1, lN - 1 - k);
+                        if (k < 2) up[6 + k] = Sv(2, lN - 1 - k);
+                    }
+                }
+                __syncthreads();
+                if (s == 0) {
+                    // a6: collapse test of PAPER.md:85 on the state after n steps (flags of every chunk)
+                    if (n > 0 && misc[2] != 0.0) { collapsed = 1; break; }
+                    if (n == prm.nsteps) break;                          // final flag round only
+                }
+                double carry = misc[0];
+                facc = 0.0; bad = 0;
+                const double a_next = K.a_next[s], b_w = K.b_w[s];
+
+                // ---- tiles, from high x to low x
+                for (int tt = ntile - 1; tt >= 0; --tt) {
+                    const int tl0 = tt * SP_TILE;
+                    const int tend = min(tl0 + SP_TILE, cn);
+                    const int l0 = tl0 + SP_PPT * tid;
+                    const int i0 = ci0 + l0;                              // global index of my first point
+                    const bool any = l0 < tend;
+                    const bool tile_hi_is_domain_end = (ci0 + tend == N); // the tile holds i = N-1
+                    const bool last_thr = any && (l0 + SP_PPT >= tend);   // owner of the tile's last point
+
+                    // stage state: ph[r], pi[r] at l0 - 3 + r (r = 0..9), a at l0..l0+3
+                    double ph[10], pi[10], a[4];
+                    if (l0 + 7 <= tend) {
+#pragma unroll
+                        for (int r = 0; r < 10; ++r) { ph[r] = Sv(0, l0 - 3 + r); pi[r] = Sv(1, l0 - 3 + r); }
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) a[q] = Sv(2, l0 + q);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < 10; ++r) { ph[r] = ldv(0, l0 - 3 + r, tend); pi[r] = ldv(1, l0 - 3 + r, tend); }
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) a[q] = ldv(2, l0 + q, tend);
+                    }
+                    // u^n and the accumulator of my points (global, prefetched; stage 0: u^n is the stage state)
+                    double un[3][4], acc[3][4];
+                    if (any && s > 0) {
+#pragma unroll
+                        for (int v = 0; v < 3; ++v) {
+                            const double2 *pa = reinterpret_cast<const double2 *>(prm.ACC[v] + row + i0);
+                            const double2 x0 = pa[0], x1 = pa[1];
+                            acc[v][0] = x0.x; acc[v][1] = x0.y; acc[v][2] = x1.x; acc[v][3] = x1.y;
+                            if (s < 3) {
+                                const double2 *pu = reinterpret_cast<const double2 *>(prm.U[v] + row + i0);
+                                const double2 y0 = pu[0], y1 = pu[1];
+                                un[v][0] = y0.x; un[v][1] = y0.y; un[v][2] = y1.x; un[v][3] = y1.y;
+                            }
+                        }
+                    }
+                    // coefficient tables of my points
+                    double m2sc[4], tT4[4], tC4[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int i = min(i0 + q, N - 1);
+                        m2sc[q] = -2.0 * tSC[i]; tT4[q] = tT[i]; tC4[q] = tC[i] * K.d4c;
+                    }
+
+                    // a1: f' = -2 sc (Phi^2 + Pi^2) of my points (zero above i = N-2 and outside the chunk)
+                    double fo[4], so[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const bool in = (l0 + q < cn) && (i0 + q <= N - 2);
+                        fo[q] = in ? m2sc[q] * fma(ph[3 + q], ph[3 + q], pi[3 + q] * pi[3 + q]) : 0.0;
+                    }
+                    const double fm = (-2.0 * tSC[min(i0 - 1, N - 1)]) * fma(ph[2], ph[2], pi[2] * pi[2]);  // f'_{l0-1}
+                    const double fp = (i0 + 4 <= N - 2) ? (-2.0 * tSC[i0 + 4]) * fma(ph[7], ph[7], pi[7] * pi[7]) : 0.0;
+                    so[3] = fo[3];
+#pragma unroll
+                    for (int q = 2; q >= 0; --q) so[q] = so[q + 1] + fo[q];
+                    // a2: tile-level suffix scan; B = sum of f' over all points above my four
+                    double ttot;
+                    const double B = block_suffix_excl_sp(so[0], sw, ttot) + carry;
+                    // -delta by the telescoped rule, E = e^{-delta}
+                    double nd[4], E[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const double f_lo = (q == 0) ? fm : fo[q - 1];
+                        const double f_hi = (q == 3) ? fp : fo[q + 1];
+                        const double s2 = (q + 2 < 4) ? so[q + 2] + B : ((q + 2 == 4) ? B : B - fp);
+                        double loc = K.c25 * f_hi;
+                        loc = fma(K.c12, fo[q], loc);
+                        loc = fma(-K.c1, f_lo, loc);
+                        nd[q] = fma(K.hh, s2, loc);
+                    }
+                    exp3_near<4>(nd, E);
+                    // a3: fluxes of my points
+                    double Hx[8], Fx[8], Gq[4], kA[4];        // Hx[k], Fx[k] at l0 - 2 + k
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const double AE = a[q] * E[q];
+                        const double Gv = AE * ph[3 + q];
+                        Gq[q] = Gv;
+                        Hx[2 + q] = AE * pi[3 + q];
+                        Fx[2 + q] = tT4[q] * Gv;
+                        kA[q] = (m2sc[q] * a[q]) * (Gv * pi[3 + q]);             // eq (4)
+                        sH[sp_pad(2 + SP_PPT * tid + q)] = Hx[2 + q];
+                        sF[sp_pad(2 + SP_PPT * tid + q)] = Fx[2 + q];
+                        if (i0 + q == N - 2) gE[2] = Gv;
+                        if (i0 + q == N - 3) gE[3] = Gv;
+                    }
+                    // fluxes at the two points below the tile (thread 0) ...
+                    if (tid == 0) {
+                        if (i0 == 0) {                       // x = 0: H even, F odd (R2)
+                            sH[sp_pad(1)] = Hx[3]; sH[sp_pad(0)] = Hx[4];
+                            sF[sp_pad(1)] = -Fx[3]; sF[sp_pad(0)] = -Fx[4];
+                        } else {
+                            const double f1 = fm;                                                             // f'_{l0-1}
+                            const double f2 = (-2.0 * tSC[i0 - 2]) * fma(ph[1], ph[1], pi[1] * pi[1]);        // f'_{l0-2}
+                            const double f3 = (-2.0 * tSC[i0 - 3]) * fma(ph[0], ph[0], pi[0] * pi[0]);        // f'_{l0-3}
+                            double l1 = K.c25 * fo[0]; l1 = fma(K.c12, f1, l1); l1 = fma(-K.c1, f2, l1);
+                            double l2 = K.c25 * f1;    l2 = fma(K.c12, f2, l2); l2 = fma(-K.c1, f3, l2);
+                            const double e1 = exp3_ref(fma(K.hh, so[1] + B, l1));
+                            const double e2 = exp3_ref(fma(K.hh, so[0] + B, l2));
+                            const double ae1 = Sv(2, l0 - 1) * e1, ae2 = Sv(2, l0 - 2) * e2;
+                            const double g1 = ae1 * ph[2], g2 = ae2 * ph[1];
+                            sH[sp_pad(1)] = ae1 * pi[2]; sH[sp_pad(0)] = ae2 * pi[1];
+                            sF[sp_pad(1)] = tT[i0 - 1] * g1; sF[sp_pad(0)] = tT[i0 - 2] * g2;
+                            if (i0 - 1 == N - 2) gE[2] = g1;
+                            if (i0 - 1 == N - 3) gE[3] = g1;
+                            if (i0 - 2 == N - 3) gE[3] = g2;
+                        }
+                    }
+                    // ... and at the two points above it (owner of the tile's last point), unless the tile
+                    // ends at x = pi/2, where readers apply the parity rule themselves
+                    if (last_thr && !tile_hi_is_domain_end) {
+                        const int le = tend - tl0 + 2;                   // scratch slot of local index tend
+                        const int ie = ci0 + tend;                       // its global index (<= N-1)
+                        if (ie == N - 1) {                   // H = 0 there; F by the limit of R5; then mirrored
+                            sH[sp_pad(le)] = 0.0;            sF[sp_pad(le)] = (16.0 * Gq[3] - Gq[2]) * K.inv12h2;
+                            sH[sp_pad(le + 1)] = -Hx[5];     sF[sp_pad(le + 1)] = Fx[5];
+                        } else {
+                            const double f1 = (ie + 1 <= N - 2) ? (-2.0 * tSC[ie + 1]) * fma(ph[8], ph[8], pi[8] * pi[8]) : 0.0;
+                            const double f2 = (ie + 2 <= N - 2) ? (-2.0 * tSC[ie + 2]) * fma(ph[9], ph[9], pi[9] * pi[9]) : 0.0;
+                            double l0v = K.c25 * f1; l0v = fma(K.c12, fp, l0v); l0v = fma(-K.c1, fo[3], l0v);
+                            double l1v = K.c25 * f2; l1v = fma(K.c12, f1, l1v); l1v = fma(-K.c1, fp, l1v);
+                            const double e0 = exp3_ref(fma(K.hh, B - fp - f1, l0v));
+                            const double e1 = exp3_ref(fma(K.hh, B - fp - f1 - f2, l1v));
+                            const double ae0 = up[6] * e0, ae1 = up[7] * e1;
+                            const double g0 = ae0 * ph[7], g1 = ae1 * ph[8];
+                            sH[sp_pad(le)] = ae0 * pi[7];     sH[sp_pad(le + 1)] = ae1 * pi[8];
+                            sF[sp_pad(le)] = tT[ie] * g0;     sF[sp_pad(le + 1)] = tT[ie + 1] * g1;
+                            if (ie == N - 3) gE[3] = g0;
+                            if (ie == N - 2) gE[2] = g0;
+                            if (ie + 1 == N - 3) gE[3] = g1;
+                            if (ie + 1 == N - 2) gE[2] = g1;
+                        }
+                    }
+                    __syncthreads();
+
+                    // a4: centred differences of H, F (neighbours from the scratch; parity rule at x = pi/2)
+                    {
+                        const int sb = SP_PPT * tid;                     // scratch slot of local index l0 - 2
+                        Hx[0] = sH[sp_pad(sb)];     Hx[1] = sH[sp_pad(sb + 1)];
+                        Fx[0] = sF[sp_pad(sb)];     Fx[1] = sF[sp_pad(sb + 1)];
+                        Hx[6] = sH[sp_pad(sb + 6)]; Hx[7] = sH[sp_pad(sb + 7)];
+                        Fx[6] = sF[sp_pad(sb + 6)]; Fx[7] = sF[sp_pad(sb + 7)];
+                        if (any && i0 + 5 >= N - 1) {        // my window l0-2 .. l0+5 reaches i = N-1
+                            const double lim = (16.0 * gE[2] - gE[3]) * K.inv12h2;   // F_{N-1} (R5)
+#pragma unroll
+                            for (int k = 2; k < 8; ++k) {
+                                const int j = i0 - 2 + k;
+                                if (j == N - 1) { Hx[k] = 0.0; Fx[k] = lim; }
+                            }
+#pragma unroll
+                            for (int k = 4; k < 8; ++k) {    // j = N, N+1: H odd, F even about x = pi/2 (R3)
+                                const int j = i0 - 2 + k;
+                                if (j == N) { Hx[k] = -Hx[k - 2]; Fx[k] = Fx[k - 2]; }
+                                if (j == N + 1) { Hx[k] = -Hx[k - 4]; Fx[k] = Fx[k - 4]; }
+                            }
+                        }
+                    }
+                    double nP[4], nQ[4], nA[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int i = i0 + q;
+                        const double dH = fma(8.0, Hx[q + 3] - Hx[q + 1], Hx[q] - Hx[q + 4]);
+                        const double dF = fma(8.0, Fx[q + 3] - Fx[q + 1], Fx[q] - Fx[q + 4]);
+                        double qP = K.kw[0] * ph[3 + q], qQ = K.kw[0] * pi[3 + q];        // Kreiss-Oliger (R6)
+#pragma unroll
+                        for (int j = 1; j <= 3; ++j) {
+                            qP = fma(K.kw[j], ph[3 + q - j] + ph[3 + q + j], qP);
+                            qQ = fma(K.kw[j], pi[3 + q - j] + pi[3 + q + j], qQ);
+                        }
+                        double kP = fma(K.d4c, dH, qP);
+                        double kQ = fma(tC4[q], dF, qQ);
+                        double kAv = kA[q];
+                        if (i == 0) {                        // eqs (7), (8); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
+                            kP = 0.0; kAv = 0.0;
+                            kQ = fma(8.0 * Gq[1] - Gq[2], K.c_org, qQ);
+                        }
+                        if (i >= N - 1) { kP = 0.0; kQ = 0.0; kAv = 0.0; }        // eqs (9)-(11)
+                        // a5: RK combine
+                        if (s == 0) {
+                            const double u0 = ph[3 + q], u1 = pi[3 + q], u2 = a[q];
+                            acc[0][q] = fma(b_w, kP, u0); acc[1][q] = fma(b_w, kQ, u1); acc[2][q] = fma(b_w, kAv, u2);
+                            nP[q] = fma(a_next, kP, u0);  nQ[q] = fma(a_next, kQ, u1);  nA[q] = fma(a_next, kAv, u2);
+                        } else if (s < 3) {
+                            acc[0][q] = fma(b_w, kP, acc[0][q]); acc[1][q] = fma(b_w, kQ, acc[1][q]); acc[2][q] = fma(b_w, kAv, acc[2][q]);
+                            nP[q] = fma(a_next, kP, un[0][q]);   nQ[q] = fma(a_next, kQ, un[1][q]);   nA[q] = fma(a_next, kAv, un[2][q]);
+                        } else {
+                            nP[q] = fma(b_w, kP, acc[0][q]); nQ[q] = fma(b_w, kQ, acc[1][q]); nA[q] = fma(b_w, kAv, acc[2][q]);
+                            if (i <= N - 1 && l0 + q < cn && !(nA[q] >= K.thr)) bad = 1;       // a6
+                        }
+                        if (i > N - 1) { nP[q] = 0.0; nQ[q] = 0.0; nA[q] = 0.0; acc[0][q] = 0.0; acc[1][q] = 0.0; acc[2][q] = 0.0; }
+                    }
+                    // old values of the tile's three lowest points: the upper halo of the next (lower) tile
+                    if (tid == 0) {
+                        up[0] = ph[3]; up[1] = ph[4]; up[2] = ph[5];
+                        up[3] = pi[3]; up[4] = pi[4]; up[5] = pi[5];
+                        up[6] = a[0];  up[7] = a[1];
+                    }
+                    if (any) {
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            if (l0 + q < cn) {
+                                Sv(0, l0 + q) = nP[q]; Sv(1, l0 + q) = nQ[q]; Sv(2, l0 + q) = nA[q];
+                                if (i0 + q <= N - 2) {       // f' of the new stage state, for the next publish
+                                    const double f = m2sc[q] * fma(nP[q], nP[q], nQ[q] * nQ[q]);
+                                    facc += f;
+                                    if (i0 + q == N - 2) misc[1] = f * (1.0 / 12.0);
+                                }
+                            }
+                        }
+                        if (s < 3) {
+#pragma unroll
+                            for (int v = 0; v < 3; ++v) {
+                                double2 *pa = reinterpret_cast<double2 *>(prm.ACC[v] + row + i0);
+                                pa[0] = make_double2(acc[v][0], acc[v][1]); pa[1] = make_double2(acc[v][2], acc[v][3]);
+                            }
+                        } else {
+                            double2 *p0 = reinterpret_cast<double2 *>(prm.U[0] + row + i0);
+                            double2 *p1 = reinterpret_cast<double2 *>(prm.U[1] + row + i0);
+                            double2 *p2 = reinterpret_cast<double2 *>(prm.U[2] + row + i0);
+                            p0[0] = make_double2(nP[0], nP[1]); p0[1] = make_double2(nP[2], nP[3]);
+                            p1[0] = make_double2(nQ[0], nQ[1]); p1[1] = make_double2(nQ[2], nQ[3]);
+                            p2[0] = make_double2(nA[0], nA[1]); p2[1] = make_double2(nA[2], nA[3]);
+                        }
+                    }
+                    carry += ttot;
+                    __syncthreads();
+                }   // tiles
+                bad = __syncthreads_or(bad);
+            }   // stages
+            if (collapsed || n == prm.nsteps) break;
+            ++n;
+            if (n == prm.nsteps && !prm.check_last) break;
+        }   // steps
+
+        if (c == 0 && tid == 0) {
+            const long long sd = rec->steps_done + n;
+            rec->steps_done = sd;
+            if (collapsed) { rec->collapsed = 1; rec->t_collapse = (double)sd * pb.dt; }
+        }
+        __syncthreads();
+    }   // members
+}
+
+
+// ------------------------------------------------------------------ host side
+// Chunks per member G and concurrent members: every CTA of a member must be co-resident (one CTA per
+// SM), a chunk holds at most SP_CAP points and at least one tile's worth (so the last chunk keeps >= 8).
+bool stream_persist_select(adsc_ctx *c)
+{
+    c->sp_ok = false;
+    if (c->dev_sms <= 0) return false;
+    const int N = c->pb.N, sms = c->dev_sms;
+    const int gmin = (N + SP_CAP - 1) / SP_CAP;
+    if (gmin > sms) return false;
+    const int per_member = sms / (c->pb.B < sms ? c->pb.B : sms);      // SMs a member can have
+    int G = per_member;
+    const int gmax = (N + SP_TILE - 1) / SP_TILE;
+    if (G > gmax) G = gmax;
+    if (G < gmin) G = gmin;
+    int Lc = ((N + G - 1) / G + 3) / 4 * 4;
+    G = (N + Lc - 1) / Lc;
+    if (Lc > SP_CAP || (G > 1 && N - (G - 1) * Lc < 8)) return false;
+    int groups = sms / G;
+    if (groups > c->pb.B) groups = c->pb.B;
+    if (groups < 1 || (size_t)groups * G > SP_MAX_CTAS) return false;
+    c->sp_G = G; c->sp_Lc = Lc; c->sp_groups = groups; c->sp_ok = true;
+    return true;
+}
+
+cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
+{
+    cudaError_t e = cudaFuncSetAttribute((const void *)k_stream_persist, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)SPLayout::bytes);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(c->ws.sp_counter, 0, sizeof(unsigned long long) * SP_MAX_CTAS, c->stream);
+    if (e != cudaSuccess) return e;
+    SPParams prm;
+    prm.pb = c->pb; prm.tb = c->tb;
+    for (int v = 0; v < 3; ++v) { prm.U[v] = c->ws.U[v]; prm.ACC[v] = c->ws.ACC[v]; }
+    prm.rec = c->ws.rec; prm.mbox = c->ws.sp_mbox; prm.counter = c->ws.sp_counter;
+    prm.nsteps = nsteps; prm.check_last = check_last;
+    prm.G = c->sp_G; prm.groups = c->sp_groups; prm.Lc = c->sp_Lc;
+    {
+        const double h = c->pb.h, dt = c->pb.dt, koc = c->pb.ko_eps / (64.0 * h);
+        SPConsts &k = prm.k;
+        k.d4c = 1.0 / (12.0 * h);
+        k.kw[0] = -20.0 * koc; k.kw[1] = 15.0 * koc; k.kw[2] = -6.0 * koc; k.kw[3] = koc;
+        k.hh = 0.5 * h; k.c25 = 25.0 * h / 48.0; k.c12 = 0.25 * h; k.c1 = h / 48.0;
+        k.inv12h2 = 1.0 / (12.0 * h * h); k.c_org = 1.0 / (2.0 * h);
+        k.a_next[0] = 0.5 * dt; k.a_next[1] = 0.5 * dt; k.a_next[2] = dt; k.a_next[3] = 0.0;
+        k.b_w[0] = dt / 6.0; k.b_w[1] = dt / 3.0; k.b_w[2] = dt / 3.0; k.b_w[3] = dt / 6.0;
+        k.thr = c->pb.thr;
+    }
+    void *args[] = { (void *)&prm };
+    e = cudaLaunchCooperativeKernel((const void *)k_stream_persist, dim3((unsigned)(c->sp_G * c->sp_groups)),
+                                    dim3(SP_THREADS), args, SPLayout::bytes, c->stream);
+    c->launches++;
+    return e;
+}
+
+}  // namespace adsc

@@ -56,7 +56,7 @@ def _bc_invariants(f):
     assert (f["delta"][:, -1] == 0).all()
 
 
-@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("path", [1, 2, 3])
 def test_set_initial_matches_oracle(env, path):
     Phi, Pi, _ = env["inputs"].make("cfg1")
     ens, f, d = _gpu_run(env, Phi, Pi, 0, path=path)
@@ -71,7 +71,7 @@ def test_set_initial_matches_oracle(env, path):
     assert d["argmin_A"][0] == od["argmin_A"][0]
 
 
-@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("path", [1, 2, 3])
 def test_cfg1_1000_steps(env, path):
     """configs[0]: N=1025, one Gaussian pulse."""
     Phi, Pi, _ = env["inputs"].make("cfg1")
@@ -91,7 +91,8 @@ def test_cfg1_1000_steps(env, path):
 
 @pytest.mark.parametrize("name,B,path,nthr", [
     ("cfg2", 8, 2, 8),     # N=4097: cluster of 2 CTAs per member
-    ("cfg2", 3, 1, 8),
+    ("cfg2", 3, 1, 8),     # persistent streaming kernel: 5 chunks per member, 3 members at once
+    ("cfg2", 3, 3, 8),     # generic streaming kernels
     ("cfg5", 8, 2, 8),     # N=2049: one CTA per member
     ("cfg3", 4, 2, 8),     # N=8193: cluster of 4
 ])
@@ -107,15 +108,31 @@ def test_config_shapes_1000_steps(env, name, B, path, nthr):
     assert np.max(np.abs(d["mass"] - od["mass"]) / np.abs(od["mass"])) <= 1e-11
 
 
-def test_streaming_many_tiles(env):
-    """Streaming path across many tiles with a ragged tail (N-1 not a tile multiple)."""
+@pytest.mark.parametrize("path", [1, 3])
+def test_streaming_many_tiles(env, path):
+    """Streaming paths across many tiles with a ragged tail (N-1 not a tile multiple)."""
     N = 65 * 1024 + 137
     N += (N + 1) % 2          # odd
     Phi, Pi, _ = env["inputs"].make("cfg4", N=N)
-    ens, f, d = _gpu_run(env, Phi, Pi, 100, path=1)
+    ens, f, d = _gpu_run(env, Phi, Pi, 100, path=path)
+    assert ens.path[0] == path
     ev = env["oracle"].Evolution(Phi, Pi).step(100)
     _compare(f, ev)
     _bc_invariants(f)
+
+
+def test_streaming_more_members_than_groups(env):
+    """Persistent streaming kernel with more members than concurrent groups: N=20481 needs 3 chunks
+    per member, so 49 members run at once and the rest in a second round; N-1 = 4*5120 makes the
+    last chunk ragged."""
+    N, B = 20481, 60
+    Phi, Pi, _ = env["inputs"].make("cfg5", B=B, N=N)
+    ens, f, d = _gpu_run(env, Phi, Pi, 40, path=1)
+    assert ens.path == (1, 3)
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=8).step(40)
+    _compare(f, ev)
+    _bc_invariants(f)
+    assert (d["steps_done"] == 40).all() and (d["collapsed"] == 0).all()
 
 
 def test_cfg4_full_size_sampled(env):
@@ -129,7 +146,7 @@ def test_cfg4_full_size_sampled(env):
     _bc_invariants(f)
 
 
-@pytest.mark.parametrize("N,path", [(9, 1), (17, 1), (33, 1), (129, 2), (1001, 1), (257, 2), (513, 1)])
+@pytest.mark.parametrize("N,path", [(9, 1), (17, 1), (33, 1), (129, 2), (1001, 1), (257, 2), (513, 1), (17, 3), (1001, 3), (1027, 1), (2051, 1)])
 def test_small_and_odd_sizes(env, N, path):
     rng = np.random.default_rng(7 + N)
     Phi, Pi, _ = env["inputs"].make("cfg5", B=5, N=N)
@@ -145,7 +162,7 @@ def test_small_and_odd_sizes(env, N, path):
 
 def test_pure_ads_exact(env):
     """P1 on the GPU: Phi=Pi=0 stays A=1, delta=0 bit-exactly on both paths."""
-    for N, path in ((1025, 2), (1025, 1), (4097, 2)):
+    for N, path in ((1025, 2), (1025, 1), (1025, 3), (4097, 2)):
         z = np.zeros((2, N))
         ens, f, d = _gpu_run(env, z, z, 50, path=path)
         assert (f["Phi"] == 0).all() and (f["Pi"] == 0).all()
@@ -153,7 +170,7 @@ def test_pure_ads_exact(env):
         assert (d["mass"] == 0).all() and (d["constraint_residual"] == 0).all()
 
 
-@pytest.mark.parametrize("path", [2, 1])
+@pytest.mark.parametrize("path", [2, 1, 3])
 def test_collapse_flags_and_times(env, path):
     """T-collapse: eps~U[30,60], sigma=1/16, N=1025; flags identical,
     collapse times within one step, frozen members identical to the oracle's."""
@@ -197,7 +214,7 @@ def test_frozen_member_is_not_advanced(env):
             assert torch.equal(f1[k][b], f2[k][b])
 
 
-@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("path", [1, 2, 3])
 def test_A_resolve_period(env, path):
     """K_A > 0 ('periodically integrating A'): same schedule as the oracle."""
     Phi, Pi, _ = env["inputs"].make("cfg1")
