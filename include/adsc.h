@@ -64,6 +64,11 @@ extern "C" {
                                           threads per CTA) to use; EINVAL if it cannot tile N.
                                           Results do not depend on it beyond rounding order.  */
 
+#define ADSC_OPT_STREAM_PPT          6  /* tuning: contiguous points per thread of the persistent
+                                          streaming kernel, 2 (512 threads per CTA) or 4 (256
+                                          threads, default).  Results do not depend on it beyond
+                                          rounding order.                                       */
+
 typedef struct adsc_ctx *adsc_handle;
 
 /* One record per member, filled by adsc_diagnostics (host memory). */

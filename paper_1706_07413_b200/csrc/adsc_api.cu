@@ -87,7 +87,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
     c->cluster = 1; c->res_cfg = -1; c->res_force = -1;
-    c->sp_ok = false; c->sp_G = 0; c->sp_groups = 0; c->sp_Lc = 0;
+    c->sp_ok = false; c->sp_G = 0; c->sp_groups = 0; c->sp_Lc = 0; c->sp_ppt = 4;
     resolve_path(c);
     return c;
 }
@@ -145,6 +145,10 @@ int adsc_set_option(adsc_handle h, int key, double value)
         }
         return ADSC_OK;
     }
+    case ADSC_OPT_STREAM_PPT:
+        if (!(value == 2.0 || value == 4.0)) return fail(h, ADSC_EINVAL, "points per thread of the streaming kernel: 2 or 4");
+        h->sp_ppt = (int)value;
+        return ADSC_OK;
     default:
         return fail(h, ADSC_EINVAL, "unknown option key");
     }

@@ -90,6 +90,7 @@ struct adsc_ctx {
     int dev_smem_optin;
     bool sp_ok;              // persistent streaming kernel usable (decided at adsc_bind)
     int sp_G, sp_groups, sp_Lc;   // chunks per member, concurrent members, points per chunk
+    int sp_ppt;              // points per thread of the persistent streaming kernel: 2 (512 threads) or 4 (256)
     std::string err;
 };
 

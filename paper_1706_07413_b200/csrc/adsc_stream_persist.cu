@@ -19,16 +19,14 @@
 
 namespace adsc {
 
-constexpr int SP_THREADS = 256;
-constexpr int SP_PPT = 4;                          // contiguous points per thread
-constexpr int SP_TILE = SP_THREADS * SP_PPT;       // 1024
+constexpr int SP_TILE = 1024;                      // points per tile = threads x contiguous points per thread
 constexpr int SP_TILES = 7;                        // tiles per chunk
 constexpr int SP_CAP = SP_TILE * SP_TILES;         // 7168 points per CTA
 constexpr int SP_HAL = 4;                          // lower halo slots of the chunk arrays (3 used)
 constexpr int SP_MBOX = 24;                        // doubles per chunk mailbox
 
-// Shared-memory index map: thread t touches 4t+q, a stride of 4 doubles; one padding double per 16
-// makes those accesses conflict-free (16 consecutive lanes fall into 16 distinct 8-byte banks).
+// Shared-memory index map: thread t touches P t + q (P = 2 or 4), a stride of P doubles; one padding
+// double per 16 makes those accesses conflict-free (16 consecutive lanes, 16 distinct 8-byte banks).
 __host__ __device__ constexpr int sp_pad(int j) { return j + (j >> 4); }
 
 struct SPLayout {
@@ -37,11 +35,13 @@ struct SPLayout {
     static constexpr int o_S = 0;                                   // [3][field]
     static constexpr int o_H = o_S + 3 * field;
     static constexpr int o_F = o_H + flux;
-    static constexpr int o_up = o_F + flux;                         // upP[3], upQ[3], upA[2]
-    static constexpr int o_sw = o_up + 8;                           // scan scratch [40]
-    static constexpr int o_gE = o_sw + 40;                          // G_1, G_2, G_{N-2}, G_{N-3}
+    static constexpr int o_up = o_F + flux;                         // [2]{upP[3], upQ[3], upA[2]} (ping-pong by tile)
+    static constexpr int o_sw = o_up + 16;                          // scan scratch [2][40] (ping-pong)
+    static constexpr int o_gE = o_sw + 80;                          // G_1, G_2, G_{N-2}, G_{N-3}
     static constexpr int o_misc = o_gE + 4;                         // carry, top, flags ... [8]
-    static constexpr int n_doubles = o_misc + 8;
+    static constexpr int o_eSC = o_misc + 8;                        // -2 sc at every tile boundary -3..+2
+    static constexpr int o_eT = o_eSC + 6 * (SP_TILES + 1);         // tan^2 x likewise
+    static constexpr int n_doubles = o_eT + 6 * (SP_TILES + 1);
     static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
 };
 
@@ -86,6 +86,7 @@ __device__ __forceinline__ double ld_cg(const double *p)
 }
 
 // Sum over the CTA (result valid in every thread).  sw: 40 doubles.
+template <int T>
 __device__ __forceinline__ double block_sum(double v, double *sw)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -96,21 +97,21 @@ __device__ __forceinline__ double block_sum(double v, double *sw)
     __syncthreads();
     double t = 0.0;
 #pragma unroll
-    for (int w = 0; w < SP_THREADS / 32; ++w) t += sw[w];
+    for (int w = 0; w < T / 32; ++w) t += sw[w];
     return t;
 }
 
 // Exclusive suffix over the threads of the CTA: sum of S over threads above this one; total in `total`.
+template <int T>
 __device__ __forceinline__ double block_suffix_excl_sp(double S, double *sw, double &total)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const double incl = warp_suffix_incl(S);
-    __syncthreads();
-    if (lane == 0) sw[warp] = incl;
+    if (lane == 0) sw[warp] = incl;          // the caller alternates between two sw buffers
     __syncthreads();
     double above = 0.0, t = 0.0;
 #pragma unroll
-    for (int w = 0; w < SP_THREADS / 32; ++w) {
+    for (int w = 0; w < T / 32; ++w) {
         const double x = sw[w];
         t += x;
         if (w > warp) above += x;
@@ -119,12 +120,15 @@ __device__ __forceinline__ double block_suffix_excl_sp(double S, double *sw, dou
     return incl - S + above;
 }
 
-__global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_constant__ SPParams prm)
+template <int P, int T>
+__global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__ SPParams prm)
 {
+    static_assert(P * T == SP_TILE && P >= 2, "a tile is 1024 points");
     using L = SPLayout;
     extern __shared__ __align__(16) double smem[];
     double *S = smem + L::o_S, *sH = smem + L::o_H, *sF = smem + L::o_F, *up = smem + L::o_up;
     double *sw = smem + L::o_sw, *gE = smem + L::o_gE, *misc = smem + L::o_misc;
+    double *eSC = smem + L::o_eSC, *eT = smem + L::o_eT;
     auto Sv = [&](int v, int l) -> double & { return S[v * L::field + sp_pad(l + SP_HAL)]; };
 
     const Problem &pb = prm.pb;
@@ -145,12 +149,20 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
 
     // value at local index l of field v, l in [tile start - 3, tend + 3): above the tile end the OLD
     // values live in `up` (the tile above has already been overwritten with the new stage state)
-    auto ldv = [&](int v, int l, int tend) -> double {
+    auto ldv = [&](int v, int l, int tend, const double *upb) -> double {
         if (l < tend) return Sv(v, l);
         const int k = l - tend;
-        if (v == 2) return (k < 2) ? up[6 + k] : 0.0;
-        return (k < 3) ? up[3 * v + k] : 0.0;
+        if (v == 2) return (k < 2) ? upb[6 + k] : 0.0;
+        return (k < 3) ? upb[3 * v + k] : 0.0;
     };
+
+    // coefficient tables around every tile boundary of the chunk (used by the two edge threads of a tile)
+    if (tid < 6 * (ntile + 1)) {
+        const int bd = tid / 6, k = tid - 6 * bd;
+        const int j = min(max(ci0 + min(bd * SP_TILE, cn) - 3 + k, -HAL), N - 1 + HAL);
+        eSC[tid] = -2.0 * tSC[j]; eT[tid] = tT[j];
+    }
+    __syncthreads();
 
     for (int b = gi; b < pb.B; b += prm.groups) {
         MemberRec *rec = prm.rec + b;
@@ -159,7 +171,7 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
 
         // ---- load the chunk; f' total of the initial state
         double facc = 0.0;
-        for (int l = tid; l < cn; l += SP_THREADS) {
+        for (int l = tid; l < cn; l += T) {
             const int i = ci0 + l;
             const double p = prm.U[0][row + i], q = prm.U[1][row + i];
             Sv(0, l) = p; Sv(1, l) = q; Sv(2, l) = prm.U[2][row + i];
@@ -178,7 +190,7 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
                 const int par = (int)(stage_ctr & 1u);
                 double *mine = mb + ((size_t)par * G + c) * SP_MBOX;
                 // ---- publish: chunk total (+ top), collapse flag, state edges
-                double tot = block_sum(facc, sw);
+                double tot = block_sum<T>(facc, sw);
                 if (owns_top) tot += misc[1];
                 if (tid == 0) { mine[0] = tot; mine[1] = bad ? 1.0 : 0.0; }
                 if (tid < 3) {
@@ -212,14 +224,15 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
                     } else {                                             // x = 0: Phi odd, Pi and A even (R2)
                         Sv(0, -1 - k) = -Sv(0, 1 + k); Sv(1, -1 - k) = Sv(1, 1 + k); Sv(2, -1 - k) = Sv(2, 1 + k);
                     }
+                    double *upt = up + 8 * ((ntile - 1) & 1);             // buffer of the chunk's top tile
                     if (c < G - 1) {
                         const double *hi = all + (size_t)(c + 1) * SP_MBOX;
-                        up[k] = ld_cg(hi + 2 + k); up[3 + k] = ld_cg(hi + 5 + k);
-                        if (k < 2) up[6 + k] = ld_cg(hi + 8 + k);
+                        upt[k] = ld_cg(hi + 2 + k); upt[3 + k] = ld_cg(hi + 5 + k);
+                        if (k < 2) upt[6 + k] = ld_cg(hi + 8 + k);
                     } else {                                             // x = pi/2: Phi even, Pi odd (R3)
                         const int lN = N - 1 - ci0;
-                        up[k] = Sv(0, lN - 1 - k); up[3 + k] = -Sv(1, lN - 1 - k);
-                        if (k < 2) up[6 + k] = Sv(2, lN - 1 - k);
+                        upt[k] = Sv(0, lN - 1 - k); upt[3 + k] = -Sv(1, lN - 1 - k);
+                        if (k < 2) upt[6 + k] = Sv(2, lN - 1 - k);
                     }
                 }
                 __syncthreads();
@@ -233,103 +246,96 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
                 const double a_next = K.a_next[s], b_w = K.b_w[s];
 
                 // ---- tiles, from high x to low x
+                double m2n[P + 2];                                            // -2 sc of my points in the coming tile
+#pragma unroll
+                for (int q = 0; q < P + 2; ++q) m2n[q] = -2.0 * tSC[min(ci0 + (ntile - 1) * SP_TILE + P * tid + q - 1, N - 1)];
                 for (int tt = ntile - 1; tt >= 0; --tt) {
                     const int tl0 = tt * SP_TILE;
                     const int tend = min(tl0 + SP_TILE, cn);
-                    const int l0 = tl0 + SP_PPT * tid;
+                    const int l0 = tl0 + P * tid;
                     const int i0 = ci0 + l0;                              // global index of my first point
                     const bool any = l0 < tend;
                     const bool tile_hi_is_domain_end = (ci0 + tend == N); // the tile holds i = N-1
-                    const bool last_thr = any && (l0 + SP_PPT >= tend);   // owner of the tile's last point
+                    const bool last_thr = any && (l0 + P >= tend);   // owner of the tile's last point
 
-                    // stage state: ph[r], pi[r] at l0 - 3 + r (r = 0..9), a at l0..l0+3
-                    double ph[10], pi[10], a[4];
-                    if (l0 + 7 <= tend) {
+                    // stage state: ph[r], pi[r] at l0 - 3 + r (r = 0..P+5), a at l0..l0+P-1
+                    const double *upb = up + 8 * (tt & 1);                // old values above this tile
+                    double ph[P + 6], pi[P + 6], a[P];
+                    if (l0 + P + 3 <= tend) {
 #pragma unroll
-                        for (int r = 0; r < 10; ++r) { ph[r] = Sv(0, l0 - 3 + r); pi[r] = Sv(1, l0 - 3 + r); }
+                        for (int r = 0; r < P + 6; ++r) { ph[r] = Sv(0, l0 - 3 + r); pi[r] = Sv(1, l0 - 3 + r); }
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) a[q] = Sv(2, l0 + q);
+                        for (int q = 0; q < P; ++q) a[q] = Sv(2, l0 + q);
                     } else {
 #pragma unroll
-                        for (int r = 0; r < 10; ++r) { ph[r] = ldv(0, l0 - 3 + r, tend); pi[r] = ldv(1, l0 - 3 + r, tend); }
+                        for (int r = 0; r < P + 6; ++r) { ph[r] = ldv(0, l0 - 3 + r, tend, upb); pi[r] = ldv(1, l0 - 3 + r, tend, upb); }
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) a[q] = ldv(2, l0 + q, tend);
+                        for (int q = 0; q < P; ++q) a[q] = ldv(2, l0 + q, tend, upb);
                     }
-                    // u^n and the accumulator of my points (global, prefetched; stage 0: u^n is the stage state)
-                    double un[3][4], acc[3][4];
-                    if (any && s > 0) {
+                    // old values of this tile's three lowest points: the upper halo of the next (lower) tile
+                    if (tid == 0) {
+                        double *upn = up + 8 * ((tt & 1) ^ 1);
+                        upn[0] = ph[3]; upn[1] = ph[4]; upn[2] = ph[5];
+                        upn[3] = pi[3]; upn[4] = pi[4]; upn[5] = pi[5];
+                        upn[6] = a[0];  upn[7] = a[1];
+                    }
+                    // coefficient tables of my points: -2 sc was fetched during the previous tile
+                    double m2sc[P], tT4[P], tC4[P];
+                    const double m2m = m2n[0], m2p = m2n[P + 1];          // -2 sc at l0 - 1 and l0 + P
 #pragma unroll
-                        for (int v = 0; v < 3; ++v) {
-                            const double2 *pa = reinterpret_cast<const double2 *>(prm.ACC[v] + row + i0);
-                            const double2 x0 = pa[0], x1 = pa[1];
-                            acc[v][0] = x0.x; acc[v][1] = x0.y; acc[v][2] = x1.x; acc[v][3] = x1.y;
-                            if (s < 3) {
-                                const double2 *pu = reinterpret_cast<const double2 *>(prm.U[v] + row + i0);
-                                const double2 y0 = pu[0], y1 = pu[1];
-                                un[v][0] = y0.x; un[v][1] = y0.y; un[v][2] = y1.x; un[v][3] = y1.y;
-                            }
-                        }
-                    }
-                    // coefficient tables of my points
-                    double m2sc[4], tT4[4], tC4[4];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const int i = min(i0 + q, N - 1);
-                        m2sc[q] = -2.0 * tSC[i]; tT4[q] = tT[i]; tC4[q] = tC[i] * K.d4c;
-                    }
+                    for (int q = 0; q < P; ++q) { m2sc[q] = m2n[1 + q]; tT4[q] = tT[min(i0 + q, N - 1)]; tC4[q] = tC[min(i0 + q, N - 1)]; }
 
                     // a1: f' = -2 sc (Phi^2 + Pi^2) of my points (zero above i = N-2 and outside the chunk)
-                    double fo[4], so[4];
+                    double fo[P], so[P];
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
+                    for (int q = 0; q < P; ++q) {
                         const bool in = (l0 + q < cn) && (i0 + q <= N - 2);
                         fo[q] = in ? m2sc[q] * fma(ph[3 + q], ph[3 + q], pi[3 + q] * pi[3 + q]) : 0.0;
                     }
-                    const double fm = (-2.0 * tSC[min(i0 - 1, N - 1)]) * fma(ph[2], ph[2], pi[2] * pi[2]);  // f'_{l0-1}
-                    const double fp = (i0 + 4 <= N - 2) ? (-2.0 * tSC[i0 + 4]) * fma(ph[7], ph[7], pi[7] * pi[7]) : 0.0;
-                    so[3] = fo[3];
+                    const double fm = m2m * fma(ph[2], ph[2], pi[2] * pi[2]);                             // f'_{l0-1}
+                    const double fp = (i0 + P <= N - 2) ? m2p * fma(ph[P + 3], ph[P + 3], pi[P + 3] * pi[P + 3]) : 0.0;   // f'_{l0+P}
+                    so[P - 1] = fo[P - 1];
 #pragma unroll
-                    for (int q = 2; q >= 0; --q) so[q] = so[q + 1] + fo[q];
+                    for (int q = P - 2; q >= 0; --q) so[q] = so[q + 1] + fo[q];
                     // a2: tile-level suffix scan; B = sum of f' over all points above my four
                     double ttot;
-                    const double B = block_suffix_excl_sp(so[0], sw, ttot) + carry;
+                    const double B = block_suffix_excl_sp<T>(so[0], sw + 40 * (tt & 1), ttot) + carry;
                     // -delta by the telescoped rule, E = e^{-delta}
-                    double nd[4], E[4];
+                    double nd[P], E[P];
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
+                    for (int q = 0; q < P; ++q) {
                         const double f_lo = (q == 0) ? fm : fo[q - 1];
-                        const double f_hi = (q == 3) ? fp : fo[q + 1];
-                        const double s2 = (q + 2 < 4) ? so[q + 2] + B : ((q + 2 == 4) ? B : B - fp);
+                        const double f_hi = (q == P - 1) ? fp : fo[q + 1];
+                        const double s2 = (q + 2 < P) ? so[q + 2] + B : ((q + 2 == P) ? B : B - fp);
                         double loc = K.c25 * f_hi;
                         loc = fma(K.c12, fo[q], loc);
                         loc = fma(-K.c1, f_lo, loc);
                         nd[q] = fma(K.hh, s2, loc);
                     }
-                    exp3_near<4>(nd, E);
+                    exp3_near<P>(nd, E);
                     // a3: fluxes of my points
-                    double Hx[8], Fx[8], Gq[4], kA[4];        // Hx[k], Fx[k] at l0 - 2 + k
+                    double Hx[P + 4], Fx[P + 4], Gq[P], kA[P];        // Hx[k], Fx[k] at l0 - 2 + k
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
+                    for (int q = 0; q < P; ++q) {
                         const double AE = a[q] * E[q];
                         const double Gv = AE * ph[3 + q];
                         Gq[q] = Gv;
                         Hx[2 + q] = AE * pi[3 + q];
                         Fx[2 + q] = tT4[q] * Gv;
                         kA[q] = (m2sc[q] * a[q]) * (Gv * pi[3 + q]);             // eq (4)
-                        sH[sp_pad(2 + SP_PPT * tid + q)] = Hx[2 + q];
-                        sF[sp_pad(2 + SP_PPT * tid + q)] = Fx[2 + q];
+                        sH[sp_pad(2 + P * tid + q)] = Hx[2 + q];
+                        sF[sp_pad(2 + P * tid + q)] = Fx[2 + q];
+                        if (i0 + q == 1) gE[0] = Gv;
+                        if (i0 + q == 2) gE[1] = Gv;
                         if (i0 + q == N - 2) gE[2] = Gv;
                         if (i0 + q == N - 3) gE[3] = Gv;
                     }
                     // fluxes at the two points below the tile (thread 0) ...
                     if (tid == 0) {
-                        if (i0 == 0) {                       // x = 0: H even, F odd (R2)
-                            sH[sp_pad(1)] = Hx[3]; sH[sp_pad(0)] = Hx[4];
-                            sF[sp_pad(1)] = -Fx[3]; sF[sp_pad(0)] = -Fx[4];
-                        } else {
+                        if (i0 != 0) {                       // (at x = 0 the reader applies the parity rule)
                             const double f1 = fm;                                                             // f'_{l0-1}
-                            const double f2 = (-2.0 * tSC[i0 - 2]) * fma(ph[1], ph[1], pi[1] * pi[1]);        // f'_{l0-2}
-                            const double f3 = (-2.0 * tSC[i0 - 3]) * fma(ph[0], ph[0], pi[0] * pi[0]);        // f'_{l0-3}
+                            const double f2 = eSC[6 * tt + 1] * fma(ph[1], ph[1], pi[1] * pi[1]);             // f'_{l0-2}
+                            const double f3 = eSC[6 * tt] * fma(ph[0], ph[0], pi[0] * pi[0]);                 // f'_{l0-3}
                             double l1 = K.c25 * fo[0]; l1 = fma(K.c12, f1, l1); l1 = fma(-K.c1, f2, l1);
                             double l2 = K.c25 * f1;    l2 = fma(K.c12, f2, l2); l2 = fma(-K.c1, f3, l2);
                             const double e1 = exp3_ref(fma(K.hh, so[1] + B, l1));
@@ -337,7 +343,7 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
                             const double ae1 = Sv(2, l0 - 1) * e1, ae2 = Sv(2, l0 - 2) * e2;
                             const double g1 = ae1 * ph[2], g2 = ae2 * ph[1];
                             sH[sp_pad(1)] = ae1 * pi[2]; sH[sp_pad(0)] = ae2 * pi[1];
-                            sF[sp_pad(1)] = tT[i0 - 1] * g1; sF[sp_pad(0)] = tT[i0 - 2] * g2;
+                            sF[sp_pad(1)] = eT[6 * tt + 2] * g1; sF[sp_pad(0)] = eT[6 * tt + 1] * g2;
                             if (i0 - 1 == N - 2) gE[2] = g1;
                             if (i0 - 1 == N - 3) gE[3] = g1;
                             if (i0 - 2 == N - 3) gE[3] = g2;
@@ -349,52 +355,73 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
                         const int le = tend - tl0 + 2;                   // scratch slot of local index tend
                         const int ie = ci0 + tend;                       // its global index (<= N-1)
                         if (ie == N - 1) {                   // H = 0 there; F by the limit of R5; then mirrored
-                            sH[sp_pad(le)] = 0.0;            sF[sp_pad(le)] = (16.0 * Gq[3] - Gq[2]) * K.inv12h2;
-                            sH[sp_pad(le + 1)] = -Hx[5];     sF[sp_pad(le + 1)] = Fx[5];
+                            sH[sp_pad(le)] = 0.0;            sF[sp_pad(le)] = (16.0 * Gq[P - 1] - Gq[P - 2]) * K.inv12h2;
+                            sH[sp_pad(le + 1)] = -Hx[P + 1]; sF[sp_pad(le + 1)] = Fx[P + 1];
                         } else {
-                            const double f1 = (ie + 1 <= N - 2) ? (-2.0 * tSC[ie + 1]) * fma(ph[8], ph[8], pi[8] * pi[8]) : 0.0;
-                            const double f2 = (ie + 2 <= N - 2) ? (-2.0 * tSC[ie + 2]) * fma(ph[9], ph[9], pi[9] * pi[9]) : 0.0;
-                            double l0v = K.c25 * f1; l0v = fma(K.c12, fp, l0v); l0v = fma(-K.c1, fo[3], l0v);
+                            const double f1 = (ie + 1 <= N - 2) ? eSC[6 * (tt + 1) + 4] * fma(ph[P + 4], ph[P + 4], pi[P + 4] * pi[P + 4]) : 0.0;
+                            const double f2 = (ie + 2 <= N - 2) ? eSC[6 * (tt + 1) + 5] * fma(ph[P + 5], ph[P + 5], pi[P + 5] * pi[P + 5]) : 0.0;
+                            double l0v = K.c25 * f1; l0v = fma(K.c12, fp, l0v); l0v = fma(-K.c1, fo[P - 1], l0v);
                             double l1v = K.c25 * f2; l1v = fma(K.c12, f1, l1v); l1v = fma(-K.c1, fp, l1v);
                             const double e0 = exp3_ref(fma(K.hh, B - fp - f1, l0v));
                             const double e1 = exp3_ref(fma(K.hh, B - fp - f1 - f2, l1v));
-                            const double ae0 = up[6] * e0, ae1 = up[7] * e1;
-                            const double g0 = ae0 * ph[7], g1 = ae1 * ph[8];
-                            sH[sp_pad(le)] = ae0 * pi[7];     sH[sp_pad(le + 1)] = ae1 * pi[8];
-                            sF[sp_pad(le)] = tT[ie] * g0;     sF[sp_pad(le + 1)] = tT[ie + 1] * g1;
+                            const double ae0 = upb[6] * e0, ae1 = upb[7] * e1;
+                            const double g0 = ae0 * ph[P + 3], g1 = ae1 * ph[P + 4];
+                            sH[sp_pad(le)] = ae0 * pi[P + 3]; sH[sp_pad(le + 1)] = ae1 * pi[P + 4];
+                            sF[sp_pad(le)] = eT[6 * (tt + 1) + 3] * g0; sF[sp_pad(le + 1)] = eT[6 * (tt + 1) + 4] * g1;
                             if (ie == N - 3) gE[3] = g0;
                             if (ie == N - 2) gE[2] = g0;
                             if (ie + 1 == N - 3) gE[3] = g1;
                             if (ie + 1 == N - 2) gE[2] = g1;
                         }
                     }
+                    // global operands of the second half (cot^2/(12h), u^n, accumulator) and -2 sc of the next
+                    // tile: issued before the barrier so that their latency overlaps it and the stencils
+                    double un[3][P], acc[3][P];
+#pragma unroll
+                    for (int q = 0; q < P + 2; ++q) m2n[q] = -2.0 * tSC[max(i0 + q - 1 - SP_TILE, -1)];
+                    if (any && s > 0) {
+#pragma unroll
+                        for (int v = 0; v < 3; ++v) {
+                            const double2 *pa = reinterpret_cast<const double2 *>(prm.ACC[v] + row + i0);
+#pragma unroll
+                            for (int q = 0; q < P; q += 2) { const double2 x = pa[q / 2]; acc[v][q] = x.x; acc[v][q + 1] = x.y; }
+                            if (s < 3) {
+                                const double2 *pu = reinterpret_cast<const double2 *>(prm.U[v] + row + i0);
+#pragma unroll
+                                for (int q = 0; q < P; q += 2) { const double2 y = pu[q / 2]; un[v][q] = y.x; un[v][q + 1] = y.y; }
+                            }
+                        }
+                    }
                     __syncthreads();
 
                     // a4: centred differences of H, F (neighbours from the scratch; parity rule at x = pi/2)
                     {
-                        const int sb = SP_PPT * tid;                     // scratch slot of local index l0 - 2
-                        Hx[0] = sH[sp_pad(sb)];     Hx[1] = sH[sp_pad(sb + 1)];
-                        Fx[0] = sF[sp_pad(sb)];     Fx[1] = sF[sp_pad(sb + 1)];
-                        Hx[6] = sH[sp_pad(sb + 6)]; Hx[7] = sH[sp_pad(sb + 7)];
-                        Fx[6] = sF[sp_pad(sb + 6)]; Fx[7] = sF[sp_pad(sb + 7)];
-                        if (any && i0 + 5 >= N - 1) {        // my window l0-2 .. l0+5 reaches i = N-1
+                        const int sb = P * tid;                          // scratch slot of local index l0 - 2
+                        Hx[0] = sH[sp_pad(sb)];             Hx[1] = sH[sp_pad(sb + 1)];
+                        Fx[0] = sF[sp_pad(sb)];             Fx[1] = sF[sp_pad(sb + 1)];
+                        Hx[P + 2] = sH[sp_pad(sb + P + 2)]; Hx[P + 3] = sH[sp_pad(sb + P + 3)];
+                        Fx[P + 2] = sF[sp_pad(sb + P + 2)]; Fx[P + 3] = sF[sp_pad(sb + P + 3)];
+                        if (i0 == 0) {                       // x = 0: H even, F odd (R2)
+                            Hx[0] = Hx[4]; Hx[1] = Hx[3]; Fx[0] = -Fx[4]; Fx[1] = -Fx[3];
+                        }
+                        if (any && i0 + P + 1 >= N - 1) {    // my window l0-2 .. l0+P+1 reaches i = N-1
                             const double lim = (16.0 * gE[2] - gE[3]) * K.inv12h2;   // F_{N-1} (R5)
 #pragma unroll
-                            for (int k = 2; k < 8; ++k) {
+                            for (int k = 2; k < P + 4; ++k) {
                                 const int j = i0 - 2 + k;
                                 if (j == N - 1) { Hx[k] = 0.0; Fx[k] = lim; }
                             }
 #pragma unroll
-                            for (int k = 4; k < 8; ++k) {    // j = N, N+1: H odd, F even about x = pi/2 (R3)
+                            for (int k = 4; k < P + 4; ++k) {    // j = N, N+1: H odd, F even about x = pi/2 (R3)
                                 const int j = i0 - 2 + k;
                                 if (j == N) { Hx[k] = -Hx[k - 2]; Fx[k] = Fx[k - 2]; }
                                 if (j == N + 1) { Hx[k] = -Hx[k - 4]; Fx[k] = Fx[k - 4]; }
                             }
                         }
                     }
-                    double nP[4], nQ[4], nA[4];
+                    double nP[P], nQ[P], nA[P];
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
+                    for (int q = 0; q < P; ++q) {
                         const int i = i0 + q;
                         const double dH = fma(8.0, Hx[q + 3] - Hx[q + 1], Hx[q] - Hx[q + 4]);
                         const double dF = fma(8.0, Fx[q + 3] - Fx[q + 1], Fx[q] - Fx[q + 4]);
@@ -405,11 +432,11 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
                             qQ = fma(K.kw[j], pi[3 + q - j] + pi[3 + q + j], qQ);
                         }
                         double kP = fma(K.d4c, dH, qP);
-                        double kQ = fma(tC4[q], dF, qQ);
+                        double kQ = fma(tC4[q] * K.d4c, dF, qQ);
                         double kAv = kA[q];
                         if (i == 0) {                        // eqs (7), (8); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
                             kP = 0.0; kAv = 0.0;
-                            kQ = fma(8.0 * Gq[1] - Gq[2], K.c_org, qQ);
+                            kQ = fma(8.0 * gE[0] - gE[1], K.c_org, qQ);
                         }
                         if (i >= N - 1) { kP = 0.0; kQ = 0.0; kAv = 0.0; }        // eqs (9)-(11)
                         // a5: RK combine
@@ -426,15 +453,9 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
                         }
                         if (i > N - 1) { nP[q] = 0.0; nQ[q] = 0.0; nA[q] = 0.0; acc[0][q] = 0.0; acc[1][q] = 0.0; acc[2][q] = 0.0; }
                     }
-                    // old values of the tile's three lowest points: the upper halo of the next (lower) tile
-                    if (tid == 0) {
-                        up[0] = ph[3]; up[1] = ph[4]; up[2] = ph[5];
-                        up[3] = pi[3]; up[4] = pi[4]; up[5] = pi[5];
-                        up[6] = a[0];  up[7] = a[1];
-                    }
                     if (any) {
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
+                        for (int q = 0; q < P; ++q) {
                             if (l0 + q < cn) {
                                 Sv(0, l0 + q) = nP[q]; Sv(1, l0 + q) = nQ[q]; Sv(2, l0 + q) = nA[q];
                                 if (i0 + q <= N - 2) {       // f' of the new stage state, for the next publish
@@ -448,19 +469,22 @@ __global__ void __launch_bounds__(SP_THREADS, 1) k_stream_persist(const __grid_c
 #pragma unroll
                             for (int v = 0; v < 3; ++v) {
                                 double2 *pa = reinterpret_cast<double2 *>(prm.ACC[v] + row + i0);
-                                pa[0] = make_double2(acc[v][0], acc[v][1]); pa[1] = make_double2(acc[v][2], acc[v][3]);
+#pragma unroll
+                                for (int q = 0; q < P; q += 2) pa[q / 2] = make_double2(acc[v][q], acc[v][q + 1]);
                             }
                         } else {
                             double2 *p0 = reinterpret_cast<double2 *>(prm.U[0] + row + i0);
                             double2 *p1 = reinterpret_cast<double2 *>(prm.U[1] + row + i0);
                             double2 *p2 = reinterpret_cast<double2 *>(prm.U[2] + row + i0);
-                            p0[0] = make_double2(nP[0], nP[1]); p0[1] = make_double2(nP[2], nP[3]);
-                            p1[0] = make_double2(nQ[0], nQ[1]); p1[1] = make_double2(nQ[2], nQ[3]);
-                            p2[0] = make_double2(nA[0], nA[1]); p2[1] = make_double2(nA[2], nA[3]);
+#pragma unroll
+                            for (int q = 0; q < P; q += 2) {
+                                p0[q / 2] = make_double2(nP[q], nP[q + 1]);
+                                p1[q / 2] = make_double2(nQ[q], nQ[q + 1]);
+                                p2[q / 2] = make_double2(nA[q], nA[q + 1]);
+                            }
                         }
                     }
                     carry += ttot;
-                    __syncthreads();
                 }   // tiles
                 bad = __syncthreads_or(bad);
             }   // stages
@@ -501,13 +525,15 @@ bool stream_persist_select(adsc_ctx *c)
     if (groups > c->pb.B) groups = c->pb.B;
     if (groups < 1 || (size_t)groups * G > SP_MAX_CTAS) return false;
     c->sp_G = G; c->sp_Lc = Lc; c->sp_groups = groups; c->sp_ok = true;
+    if (c->sp_ppt != 2 && c->sp_ppt != 4) c->sp_ppt = 4;
     return true;
 }
 
 cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
 {
-    cudaError_t e = cudaFuncSetAttribute((const void *)k_stream_persist, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)SPLayout::bytes);
+    const void *fn = c->sp_ppt == 4 ? (const void *)k_stream_persist<4, 256> : (const void *)k_stream_persist<2, 512>;
+    const int threads = SP_TILE / c->sp_ppt;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SPLayout::bytes);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(c->ws.sp_counter, 0, sizeof(unsigned long long) * SP_MAX_CTAS, c->stream);
     if (e != cudaSuccess) return e;
@@ -529,8 +555,8 @@ cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
         k.thr = c->pb.thr;
     }
     void *args[] = { (void *)&prm };
-    e = cudaLaunchCooperativeKernel((const void *)k_stream_persist, dim3((unsigned)(c->sp_G * c->sp_groups)),
-                                    dim3(SP_THREADS), args, SPLayout::bytes, c->stream);
+    e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)(c->sp_G * c->sp_groups)), dim3((unsigned)threads), args,
+                                    SPLayout::bytes, c->stream);
     c->launches++;
     return e;
 }

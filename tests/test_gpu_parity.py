@@ -108,13 +108,13 @@ def test_config_shapes_1000_steps(env, name, B, path, nthr):
     assert np.max(np.abs(d["mass"] - od["mass"]) / np.abs(od["mass"])) <= 1e-11
 
 
-@pytest.mark.parametrize("path", [1, 3])
-def test_streaming_many_tiles(env, path):
+@pytest.mark.parametrize("path,ppt", [(1, 2), (1, 4), (3, None)])
+def test_streaming_many_tiles(env, path, ppt):
     """Streaming paths across many tiles with a ragged tail (N-1 not a tile multiple)."""
     N = 65 * 1024 + 137
     N += (N + 1) % 2          # odd
     Phi, Pi, _ = env["inputs"].make("cfg4", N=N)
-    ens, f, d = _gpu_run(env, Phi, Pi, 100, path=path)
+    ens, f, d = _gpu_run(env, Phi, Pi, 100, path=path, stream_ppt=ppt)
     assert ens.path[0] == path
     ev = env["oracle"].Evolution(Phi, Pi).step(100)
     _compare(f, ev)
@@ -146,14 +146,16 @@ def test_cfg4_full_size_sampled(env):
     _bc_invariants(f)
 
 
-@pytest.mark.parametrize("N,path", [(9, 1), (17, 1), (33, 1), (129, 2), (1001, 1), (257, 2), (513, 1), (17, 3), (1001, 3), (1027, 1), (2051, 1)])
-def test_small_and_odd_sizes(env, N, path):
+@pytest.mark.parametrize("N,path,ppt", [(9, 1, 2), (17, 1, 4), (33, 1, 2), (129, 2, None), (1001, 1, 2), (257, 2, None),
+                                        (513, 1, 4), (17, 3, None), (1001, 3, None), (1027, 1, 2), (1027, 1, 4),
+                                        (2051, 1, 2), (2051, 1, 4)])
+def test_small_and_odd_sizes(env, N, path, ppt):
     rng = np.random.default_rng(7 + N)
     Phi, Pi, _ = env["inputs"].make("cfg5", B=5, N=N)
     x = env["inputs"].grid(N)
     Phi = 0.05 * rng.uniform(0.5, 1.0, (5, 1)) * np.sin(2 * x)[None, :] * np.cos(x)[None, :] ** 2
     Phi[:, 0] = 0; Phi[:, -1] = 0
-    ens, f, d = _gpu_run(env, Phi, Pi, 300, path=path)
+    ens, f, d = _gpu_run(env, Phi, Pi, 300, path=path, stream_ppt=ppt)
     assert ens.path[0] == path
     ev = env["oracle"].Evolution(Phi, Pi).step(300)
     _compare(f, ev)
