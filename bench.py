@@ -36,6 +36,10 @@ BYTES_PER_POINT_STEP = 384.0
 # measured DFMA issue rate on this pool is recorded there too).
 FP64_LANES_PER_SM = 64
 N_SMS = 148
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE stage-kernel launch from the committed `ncu --set full`
+# captures (profiles/r01_summary.md).  The state is loaded and stored once per launch whatever the number of
+# RK4 steps in it (resident path) or stays L2-resident (cfg4), so the figure does not scale with rk4_per_step.
+NCU_TRAFFIC_BYTES = {"cfg2": 150.1e6, "cfg5": 1564.9e6, "cfg3": 1561.0e6, "cfg4": 264.5e6, "cfg1": None}
 
 
 def parse():
@@ -47,7 +51,7 @@ def parse():
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--rk4-per-step", type=int, default=0, help="RK4 steps per bench step (0 = workload default)")
     ap.add_argument("--batch", type=int, default=0, help="override the ensemble size (0 = workload default)")
-    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 streaming, 2 resident")
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 persistent streaming, 2 resident, 3 generic streaming")
     ap.add_argument("--variant", type=int, default=None, help="resident kernel variant (tuning; default auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
@@ -291,16 +295,20 @@ def main():
         peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
         ach_tf = per_gpu_rate * SLOTS_PER_POINT_STEP * 2 / 1e12
         roof = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach_tf / peak_tf, "traffic": None,
-                "kernel": "k_resident (whole RK4 steps on chip; 1 launch per adsc_step)",
+                "frac": ach_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(name) if B == cfg["B"] else None,
+                "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
+                "kernel": "k_resident3 (whole RK4 steps on chip; 1 launch per adsc_step)",
                 "peak_src": f"derived: {N_SMS} SMs x {FP64_LANES_PER_SM} DFMA lanes x "
                             f"{peaks['sm_max_mhz']:.0f} MHz x 2 flop (DESIGN.md Roofline)",
                 "algorithmic": f"{SLOTS_PER_POINT_STEP:.0f} FP64-pipe instr per point per RK4 step"}
     else:
         ach = per_gpu_rate * BYTES_PER_POINT_STEP / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"], "traffic": None,
-                "kernel": "k_stream_* (4 stage passes per RK4 step)",
+                "frac": ach / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(name) if B == cfg["B"] else None,
+                "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
+                "kernel": ("k_stream_persist (stage state in shared memory, u^n/accumulator through L2; "
+                           "1 cooperative launch per adsc_step)" if path == 1 else
+                           "k_stream_rhs (+ k_stream_I, k_stream_carry: 3 launches per RK stage)"),
                 "peak_src": f"{peaks['src']} copy bandwidth (MEASURED_PEAKS.json)",
                 "algorithmic": f"{BYTES_PER_POINT_STEP:.0f} B per point per RK4 step"}
 
@@ -314,7 +322,8 @@ def main():
         "dtype": "f64", "data": "synthetic (seeded, paper_1706_07413_b200/inputs.py)",
         "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_per_gpu": B, "global_batch": B * world,
                    "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1,
-                   "path": {1: "streaming", 2: "resident"}[path], "ctas_per_member": cluster,
+                   "path": {1: "streaming-persistent", 2: "resident", 3: "streaming-generic"}[path],
+                   "ctas_per_member": cluster,
                    "parallelism": f"members sharded over {world} GPU(s), no collective",
                    "l2": "flushed between timed iterations (256 MiB fill)",
                    "active_fraction": active_frac},
