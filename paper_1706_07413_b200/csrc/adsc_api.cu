@@ -31,6 +31,9 @@ static void compute_layout(adsc_ctx *c)
     L.off_Ac = off; off += field;
     L.off_tot = off; off += stream ? tiles : 0;
     L.off_carry = off; off += stream ? tiles : 0;
+    L.off_tot2 = off; off += stream ? tiles : 0;
+    L.off_carry2 = off; off += stream ? tiles : 0;
+    L.off_part = off; off += stream ? 6 * tiles : 0;
     for (int k = 0; k < 2; ++k) { L.off_stage[k] = off; off += ext; }
     L.off_tab = off; off += align_up((size_t)5 * (c->pb.NP + 2 * HAL) * sizeof(double), 256);
     L.off_rec = off; off += align_up((size_t)c->pb.B * sizeof(MemberRec), 256);
@@ -181,6 +184,9 @@ int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream)
     h->ws.Ac = (double *)(base + L.off_Ac);
     h->ws.tot = (double *)(base + L.off_tot);
     h->ws.carry = (double *)(base + L.off_carry);
+    h->ws.tot2 = (double *)(base + L.off_tot2);
+    h->ws.carry2 = (double *)(base + L.off_carry2);
+    h->ws.part = (double *)(base + L.off_part);
     h->ws.stage[0] = (double *)(base + L.off_stage[0]);
     h->ws.stage[1] = (double *)(base + L.off_stage[1]);
     h->ws.tab = (double *)(base + L.off_tab);

@@ -53,6 +53,8 @@ struct Workspace {
     double *Ac;          // scratch: A from eq (5) (diagnostics)
     double *tot;         // streaming: [B][ntiles] tile totals
     double *carry;       // streaming: [B][ntiles] exclusive suffix of tot
+    double *tot2, *carry2;   // tiled constraint solve: tile totals / exclusive prefix of the A integrand
+    double *part;        // tiled constraint solve: [B][ntiles][6] diagnostics partials
     double *stage[2];    // host staging [B][N]
     double *sp_mbox;     // persistent streaming: [SP_MAX_CTAS][2][24] chunk mailboxes
     unsigned long long *sp_counter;   // persistent streaming: [SP_MAX_CTAS] group barrier counters
@@ -61,7 +63,7 @@ struct Workspace {
 };
 
 struct Layout {
-    size_t off_U[3], off_Ua[3], off_Ub[3], off_ACC[3], off_dl, off_Ac, off_tot, off_carry,
+    size_t off_U[3], off_Ua[3], off_Ub[3], off_ACC[3], off_dl, off_Ac, off_tot, off_carry, off_tot2, off_carry2, off_part,
         off_stage[2], off_tab, off_rec, off_mbox, off_cnt, total;
     int ntiles;
 };
@@ -102,7 +104,9 @@ cudaError_t launch_pack(adsc_ctx *c, const double *src, int field, bool init_rec
 cudaError_t launch_unpack(adsc_ctx *c, const double *src_internal, double *dst);
 // mode bits for launch_solve
 enum { SOLVE_WRITE_A = 1, SOLVE_DIAG = 2, SOLVE_ACTIVE_ONLY = 4 };
-cudaError_t launch_solve(adsc_ctx *c, int mode);
+cudaError_t launch_solve(adsc_ctx *c, int mode);              // one CTA per member, or the tiled kernels for long members
+cudaError_t launch_solve_tiled(adsc_ctx *c, int mode);        // adsc_solve_tiled.cu (streaming layouts only)
+constexpr int SOLVE_TILED_MIN_N = 32768;                      // members at least this long use the tiled solve
 cudaError_t launch_finalize(adsc_ctx *c, int inc_steps);
 cudaError_t launch_stream_step(adsc_ctx *c);                 // one RK4 step, generic streaming kernels
 bool stream_persist_select(adsc_ctx *c);                     // fills c->sp_* (needs c->dev_sms)

@@ -357,13 +357,11 @@ static const ResConfig g_cfgs1[] = {
 };
 constexpr int n_cfgs1 = sizeof(g_cfgs1) / sizeof(g_cfgs1[0]);
 
-// Variant index space: generation 3 (preferred), then generation 2, then generation 1.
-static int n_cfgs() { return n_cfgs3 + n_cfgs2 + n_cfgs1; }
+// Variant index space: generation 3 (preferred), then generation 1 (any cluster size 2..8).
+static int n_cfgs() { return n_cfgs3 + n_cfgs1; }
 static const ResConfig &cfg_at(int k)
 {
-    if (k < n_cfgs3) return g_cfgs3[k];
-    k -= n_cfgs3;
-    return k < n_cfgs2 ? g_cfgs2[k] : g_cfgs1[k - n_cfgs2];
+    return k < n_cfgs3 ? g_cfgs3[k] : g_cfgs1[k - n_cfgs3];
 }
 static const void *fn_for(const ResConfig &g, int cl)
 {

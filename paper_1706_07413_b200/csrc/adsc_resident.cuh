@@ -42,9 +42,7 @@ struct ResConfig {
     const void *fn[4];
 };
 
-// generation-2 table (adsc_resident2.cu), generation-3 table (adsc_resident3.cu)
-extern const ResConfig g_cfgs2[];
-extern const int n_cfgs2;
+// generation-3 table (adsc_resident3.cu); the generation-1 table is local to adsc_resident.cu
 extern const ResConfig g_cfgs3[];
 extern const int n_cfgs3;
 

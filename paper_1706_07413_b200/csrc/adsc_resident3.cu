@@ -1,8 +1,10 @@
 // adsc_resident3.cu — resident RK4 kernel, third generation ("v3"): one ensemble member per CTA
 // (or per cluster of CL CTAs), the whole state on chip across all RK stages and steps.
 //
-// Arithmetic per stage is that of adsc_resident2.cu (telescoped delta rule, two synchronisation
-// points per RK stage, near-exp).  What changed, and why (profiles/r01_v2_resident.md):
+// Arithmetic per stage: telescoped delta rule, two synchronisation points per RK
+// stage, one full exp per thread and short relative polynomials for the other points.  What changed
+// against the earlier generations (generation 1 is adsc_resident.cu; generation 2, same arithmetic with
+// cluster barriers, was removed), and why:
 //   * Synchronisation is point-to-point.  Every sync point is an mbarrier in each CTA's shared memory:
 //     one elected lane per warp arrives on it (split arrive / wait, so the independent arithmetic
 //     placed between them overlaps the skew between warps also inside ONE CTA), and data for other

@@ -292,6 +292,7 @@ k_solve(Problem pb, Tables tb, const double *__restrict__ gPhi, const double *__
 
 cudaError_t launch_solve(adsc_ctx *c, int mode)
 {
+    if (c->path != 2 && c->pb.N >= SOLVE_TILED_MIN_N) return launch_solve_tiled(c, mode);
     k_solve<<<c->pb.B, SOLVE_THREADS, 0, c->stream>>>(c->pb, c->tb, c->ws.U[0], c->ws.U[1], c->ws.U[2],
                                                      c->ws.dl, c->ws.Ac, c->ws.rec, mode);
     c->launches++;

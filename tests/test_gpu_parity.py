@@ -119,6 +119,26 @@ def test_streaming_many_tiles(env, path, ppt):
     ev = env["oracle"].Evolution(Phi, Pi).step(100)
     _compare(f, ev)
     _bc_invariants(f)
+    od = ev.diagnostics()          # N >= 32768: the tiled constraint solve (adsc_solve_tiled.cu) made these
+    assert abs(d["mass"][0] - od["mass"][0]) <= 1e-11 * abs(od["mass"][0])
+    assert abs(d["constraint_residual"][0] - od["resid"][0]) <= 1e-12
+    assert abs(d["min_A"][0] - od["min_A"][0]) <= TOL and d["argmin_A"][0] == od["argmin_A"][0]
+
+
+@pytest.mark.parametrize("path", [1, 3])
+def test_long_member_A_resolve_and_set_initial(env, path):
+    """Tiled constraint solve: set_initial and the periodic A re-solve (K_A = 8) on two long members."""
+    N, B = 40961, 2
+    Phi, Pi, _ = env["inputs"].make("cfg5", B=B, N=N)
+    Pi = Pi * 8.0
+    ens, f0, d0 = _gpu_run(env, Phi, Pi, 0, path=path)
+    o0 = env["oracle"].set_initial(Phi, Pi)
+    assert np.max(np.abs(f0["A"] - o0["A"])) <= 1e-13 and np.max(np.abs(f0["delta"] - o0["delta"])) <= 1e-13
+    ens, f, d = _gpu_run(env, Phi, Pi, 40, path=path, a_resolve_period=8)
+    ev = env["oracle"].Evolution(Phi, Pi, K_A=8, nthreads=2).step(40)
+    _compare(f, ev)
+    _bc_invariants(f)
+    assert (d["constraint_residual"] < 1e-12).all()
 
 
 def test_streaming_more_members_than_groups(env):
