@@ -95,6 +95,16 @@ def rhs(Phi, Pi, A, ko_eps: float):
     return kP, kQ, kA, d
 
 
+def rhs_fixed(Phi, Pi, ko_eps: float):
+    """Right-hand side on the fixed background A = 1, delta = 0."""
+    Phi, Pi = _f64(Phi), _f64(Pi)
+    A = np.ones_like(Phi)
+    kP, kQ, kA, d = (np.zeros_like(Phi) for _ in range(4))
+    assert lib().oracle_rhs_fixed(C.c_int(Phi.size), C.c_double(ko_eps), _p(Phi), _p(Pi), _p(A),
+                                  _p(kP), _p(kQ), _p(kA), _p(d)) == 0
+    return kP, kQ, kA, d
+
+
 def set_initial(Phi, Pi):
     """[B][N] (or [N]) -> dict of Phi, Pi (Dirichlet-forced copies), A, delta."""
     Phi = np.array(np.atleast_2d(Phi), dtype=np.float64, order="C")
@@ -120,9 +130,12 @@ class Evolution:
     """A batch evolved by the oracle: state in numpy, stepped in place."""
 
     def __init__(self, Phi, Pi, courant: float = 0.25, ko_eps: float = 0.1,
-                 thr: float = 2.0 ** -7, K_A: int = 0, nthreads: int = 1):
+                 thr: float = 2.0 ** -7, K_A: int = 0, nthreads: int = 1, fixed_background: bool = False):
         s = set_initial(Phi, Pi)
         self.Phi, self.Pi, self.A = s["Phi"], s["Pi"], s["A"]
+        self.fixed_background = bool(fixed_background)
+        if self.fixed_background:          # PAPER.md:177: A and delta held fixed at 1 and 0
+            self.A = np.ones_like(self.Phi)
         self.B, self.N = self.Phi.shape
         self.courant, self.ko_eps, self.thr, self.K_A = courant, ko_eps, thr, K_A
         self.nthreads = nthreads
@@ -133,6 +146,15 @@ class Evolution:
         self.t_collapse = np.full(self.B, np.nan)
 
     def step(self, nsteps: int):
+        if self.fixed_background:
+            r = lib().oracle_evolve_fixed(
+                C.c_int(self.N), C.c_int(self.B), C.c_double(self.courant), C.c_double(self.ko_eps),
+                C.c_longlong(nsteps), _p(self.Phi), _p(self.Pi), _p(self.A),
+                self.steps_done.ctypes.data_as(C.POINTER(C.c_longlong)),
+                self.collapsed.ctypes.data_as(C.POINTER(C.c_int)), _p(self.t_collapse),
+                C.c_int(self.nthreads))
+            assert r == 0
+            return self
         r = lib().oracle_evolve(
             C.c_int(self.N), C.c_int(self.B), C.c_double(self.courant), C.c_double(self.ko_eps),
             C.c_double(self.thr), C.c_int(self.K_A), C.c_longlong(nsteps),
@@ -145,6 +167,8 @@ class Evolution:
 
     @property
     def delta(self):
+        if self.fixed_background:
+            return np.zeros_like(self.Phi)
         return np.stack([delta_solve(self.Phi[b], self.Pi[b]) for b in range(self.B)])
 
     def diagnostics(self):

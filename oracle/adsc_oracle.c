@@ -173,13 +173,17 @@ static void A_solve(const tables *tb, const double *Phi, const double *Pi,
  * held by zero rhs. */
 typedef struct { double *delta, *f, *G, *H, *F; } rhs_ws;
 
-static void rhs(const tables *tb, double ko_eps, const double *Phi, const double *Pi,
+/* fixed_bg != 0 is the paper's second workload (Table II: "both A and delta are not
+ * dynamical i.e. held fixed at 1 and 0 respectively"): delta = 0 is not integrated, the A passed in
+ * (A = 1 from set_initial) is used as it is and not evolved (kA = 0).  (SURVEY.md 8(f) f1.) */
+static void rhs(const tables *tb, double ko_eps, int fixed_bg, const double *Phi, const double *Pi,
                 const double *A, double *kPhi, double *kPi, double *kA, rhs_ws *ws)
 {
     const int N = tb->N;
     const double h = tb->h;
     double *delta = ws->delta, *G = ws->G, *H = ws->H, *F = ws->F;
-    delta_solve(tb, Phi, Pi, delta, ws->f);
+    if (fixed_bg) { for (int i = 0; i < N; ++i) delta[i] = 0.0; }
+    else delta_solve(tb, Phi, Pi, delta, ws->f);
     for (int i = 0; i < N; ++i) {
         double E = exp(-delta[i]);
         double AE = A[i] * E;
@@ -196,7 +200,7 @@ static void rhs(const tables *tb, double ko_eps, const double *Phi, const double
             kPi[i] = tb->C[i] * D4(F, N, h, i, -1, +1) + KO(Pi, N, h, ko_eps, i, +1, -1);
         else
             kPi[i] = 0.0;
-        kA[i] = -2.0 * tb->sc[i] * A[i] * G[i] * Pi[i];
+        kA[i] = fixed_bg ? 0.0 : -2.0 * tb->sc[i] * A[i] * G[i] * Pi[i];
     }
     kPhi[0] = 0.0; kPhi[N - 1] = 0.0; kPi[N - 1] = 0.0; kA[0] = 0.0; kA[N - 1] = 0.0;
 }
@@ -206,6 +210,7 @@ static void rhs(const tables *tb, double ko_eps, const double *Phi, const double
 typedef struct {
     tables tb;
     double ko_eps, dt;
+    int fixed_bg;      /* A = 1, delta = 0 held fixed */
     rhs_ws ws;
     double *k[3];      /* current stage slope of (Phi, Pi, A)   */
     double *us[3];     /* stage state u*                         */
@@ -252,7 +257,7 @@ static void rk4_step(stepper *st, double *Phi, double *Pi, double *A)
         memset(st->acc[v], 0, N * sizeof(double));
     }
     for (int s = 0; s < 4; ++s) {
-        rhs(&st->tb, st->ko_eps, st->us[0], st->us[1], st->us[2],
+        rhs(&st->tb, st->ko_eps, st->fixed_bg, st->us[0], st->us[1], st->us[2],
             st->k[0], st->k[1], st->k[2], &st->ws);
         for (int v = 0; v < 3; ++v)
             for (int i = 0; i < N; ++i) {
@@ -340,7 +345,18 @@ int oracle_rhs(int N, double ko_eps, const double *Phi, const double *Pi, const 
                double *kPhi, double *kPi, double *kA, double *delta)
 {
     stepper st; if (stepper_init(&st, N, 0.25, ko_eps)) return -1;
-    rhs(&st.tb, ko_eps, Phi, Pi, A, kPhi, kPi, kA, &st.ws);
+    rhs(&st.tb, ko_eps, 0, Phi, Pi, A, kPhi, kPi, kA, &st.ws);
+    memcpy(delta, st.ws.delta, N * sizeof(double));
+    stepper_free(&st);
+    return 0;
+}
+
+/* The same on the fixed background A = 1, delta = 0 of PAPER.md:177 (A is an input: pass ones). */
+int oracle_rhs_fixed(int N, double ko_eps, const double *Phi, const double *Pi, const double *A,
+               double *kPhi, double *kPi, double *kA, double *delta)
+{
+    stepper st; if (stepper_init(&st, N, 0.25, ko_eps)) return -1;
+    rhs(&st.tb, ko_eps, 1, Phi, Pi, A, kPhi, kPi, kA, &st.ws);
     memcpy(delta, st.ws.delta, N * sizeof(double));
     stepper_free(&st);
     return 0;
@@ -397,7 +413,7 @@ int oracle_diagnostics(int N, int B, const double *Phi, const double *Pi, const 
  * steps_done / collapsed / t_collapse are in-out per-member arrays (a fresh
  * run passes zeros / zeros / NaN).  nthreads>1 runs members in parallel
  * (members are independent; the scans stay serial inside a member). */
-int oracle_evolve(int N, int B, double courant, double ko_eps, double thr, int K_A,
+static int evolve(int N, int B, double courant, double ko_eps, double thr, int K_A, int fixed_bg,
                   long long nsteps, double *Phi, double *Pi, double *A,
                   long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
 {
@@ -409,6 +425,7 @@ int oracle_evolve(int N, int B, double courant, double ko_eps, double thr, int K
     {
         stepper st;
         int ok = (stepper_init(&st, N, courant, ko_eps) == 0);
+        st.fixed_bg = fixed_bg;
         if (!ok) {
 #ifdef _OPENMP
 #pragma omp atomic write
@@ -424,7 +441,7 @@ int oracle_evolve(int N, int B, double courant, double ko_eps, double thr, int K
             for (long long n = 0; n < nsteps && !collapsed[b]; ++n) {
                 rk4_step(&st, ph, pi, a);
                 steps_done[b] += 1;
-                if (K_A > 0 && steps_done[b] % K_A == 0) {
+                if (!fixed_bg && K_A > 0 && steps_done[b] % K_A == 0) {
                     delta_solve(&st.tb, ph, pi, st.ws.delta, st.scratch);
                     A_solve(&st.tb, ph, pi, st.ws.delta, a, st.scratch);
                 }
@@ -437,6 +454,22 @@ int oracle_evolve(int N, int B, double courant, double ko_eps, double thr, int K
         if (ok) stepper_free(&st);
     }
     return err;
+}
+
+int oracle_evolve(int N, int B, double courant, double ko_eps, double thr, int K_A,
+                  long long nsteps, double *Phi, double *Pi, double *A,
+                  long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
+{
+    return evolve(N, B, courant, ko_eps, thr, K_A, 0, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
+}
+
+/* Evolution on the fixed background A = 1, delta = 0 (Table II): A is passed
+ * in (ones) and comes back unchanged, so the collapse test never fires. */
+int oracle_evolve_fixed(int N, int B, double courant, double ko_eps,
+                        long long nsteps, double *Phi, double *Pi, double *A,
+                        long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
+{
+    return evolve(N, B, courant, ko_eps, 0.0, 0, 1, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
 }
 
 int oracle_max_threads(void)

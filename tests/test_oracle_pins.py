@@ -362,3 +362,73 @@ def test_A_resolve_period_keeps_constraint_tight():
     tight = oracle.Evolution(np.zeros_like(Pi), Pi, K_A=16).step(512).diagnostics()
     assert tight["resid"][0] < 1e-13 and free["resid"][0] > 1e-9
     assert abs(tight["mass"][0] / free["mass"][0] - 1) < 1e-5
+
+
+# ------------------------------------------------- f1: fixed background A = 1, delta = 0
+
+@pytest.mark.parametrize("j", [0, 2])
+def test_F1_fixed_background_rhs_is_the_linear_operator(j):
+    # With A = 1, delta = 0 held fixed (Table II) eqs (2), (3) are exactly linear:
+    # Phi_dot = Pi', Pi_dot = tan^-2 (tan^2 Phi)'.  At FINITE amplitude the AdS4 eigenmodes must come out
+    # (omega_j = 3+2j, closed_forms.txt) with no O(eps^2) remainder, and superposition must hold to rounding.
+    om = _golden("closed_forms.txt")[f"omega_{j}"]
+    errs = []
+    for N in (129, 257, 513):
+        x = inputs.grid(N)
+        e, de = inputs.eigenmode(j, x)
+        de[0] = de[-1] = 0.0; e[-1] = 0.0
+        kP, kQ, kA, d = oracle.rhs_fixed(de, np.zeros(N), 0.0)
+        assert (kA == 0).all() and (d == 0).all()
+        errs.append(np.abs(kQ + om ** 2 * e)[N // 4:].max())
+        kP, kQ, kA, d = oracle.rhs_fixed(np.zeros(N), e, 0.0)
+        assert np.abs(kP - de).max() < 3e-3 * (129.0 / N) ** 4 * (1 + j) ** 5
+    assert errs[0] / errs[1] > 12 and errs[1] / errs[2] > 12, errs
+    N = 257
+    x = inputs.grid(N)
+    rng = np.random.default_rng(5)
+    u1, u2 = (np.sin(2 * x) * np.cos(x) ** 2 * rng.uniform(0.5, 2.0) for _ in range(2))
+    v1, v2 = (np.cos(x) ** 3 * rng.uniform(0.5, 2.0) * np.cos(3 * x) for _ in range(2))
+    for u in (u1, u2): u[0] = u[-1] = 0.0
+    for v in (v1, v2): v[-1] = 0.0
+    r1 = oracle.rhs_fixed(u1, v1, 0.1); r2 = oracle.rhs_fixed(u2, v2, 0.1)
+    r12 = oracle.rhs_fixed(2.5 * u1 - 0.75 * u2, 2.5 * v1 - 0.75 * v2, 0.1)
+    for k in (0, 1):
+        lin = 2.5 * r1[k] - 0.75 * r2[k]
+        assert np.abs(r12[k] - lin).max() <= 1e-12 * max(1.0, np.abs(lin).max())
+
+
+def test_F2_fixed_background_evolution_periodic_linear_and_conservative():
+    # Finite-amplitude single mode on the fixed background: exact periodicity of the continuum solution
+    # (all omega_j odd: Phi(pi) = -Phi(0)), exact amplitude independence (linearity of every step),
+    # A = 1 and delta = 0 untouched, no collapse, and the linear energy int tan^2 (Phi^2+Pi^2) conserved.
+    j, N = 1, 257
+    x = inputs.grid(N); tb = oracle.tables(N)
+    e, de = inputs.eigenmode(j, x)
+    Phi0 = de.copy(); Phi0[0] = Phi0[-1] = 0.0
+    steps_pi = 8 * (N - 1)
+    big = oracle.Evolution(Phi0, np.zeros(N), fixed_background=True)
+    small = oracle.Evolution(1e-3 * Phi0, np.zeros(N), fixed_background=True)
+    E0 = (tb["w"][:-1] * tb["T"][:-1] * (big.Phi[0][:-1] ** 2 + big.Pi[0][:-1] ** 2)).sum()
+    big.step(steps_pi); small.step(steps_pi)
+    flip = np.abs(big.Phi[0] + Phi0).max() / np.abs(Phi0).max()
+    assert flip < 4e-5 * (129.0 / N) ** 3 * (5 / 5.0) ** 4 + 3e-6, flip
+    assert np.abs(big.Phi[0] * 1e-3 - small.Phi[0]).max() <= 1e-12 * 1e-3 * np.abs(Phi0).max()
+    assert np.abs(big.Pi[0] * 1e-3 - small.Pi[0]).max() <= 1e-12 * 1e-3 * 5.0 * np.abs(e).max()   # |Pi| <= omega |e|
+    assert (big.A == 1).all() and (big.delta == 0).all() and not big.collapsed.any()
+    E1 = (tb["w"][:-1] * tb["T"][:-1] * (big.Phi[0][:-1] ** 2 + big.Pi[0][:-1] ** 2)).sum()
+    assert abs(E1 / E0 - 1.0) < 1e-6, (E0, E1)
+    assert abs(E0 - 25.0) < 1e-3          # omega_1^2 a^2 = 25 for a = 1 (R19 normalisation, P10)
+
+
+def test_F3_dynamical_evolution_tends_to_fixed_background_as_amplitude_vanishes():
+    # The back-reaction is O(eps^2) (delta, 1-A ~ eps^2): (Phi_dyn - Phi_fixed)/eps = O(eps^2).
+    N = 129
+    x = inputs.grid(N)
+    e, de = inputs.eigenmode(0, x)
+    Phi0 = de.copy(); Phi0[0] = Phi0[-1] = 0.0
+    d = []
+    for eps in (1e-2, 1e-3):
+        dyn = oracle.Evolution(eps * Phi0, np.zeros(N)).step(400)
+        fix = oracle.Evolution(eps * Phi0, np.zeros(N), fixed_background=True).step(400)
+        d.append(np.abs(dyn.Phi[0] - fix.Phi[0]).max() / eps)
+    assert d[0] < 1e-2 and 50 < d[0] / d[1] < 200, d
