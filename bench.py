@@ -30,6 +30,9 @@ UNIT = "updates/s"
 #   resident regime: FP64-pipe instruction slots (FMA/ADD/MUL = 1 slot); reported as
 #   TFLOP/s with 2 flop per slot so that it is commensurate with the DFMA peak.
 SLOTS_PER_POINT_STEP = 250.0
+#   fixed background: no f, scan, exp, A update: per stage fluxes 3 + D4 H 4 +
+#   cot^2 D4 F 5 + 2 x KO 14 + RK combine of Phi, Pi 4 = 30, x 4 stages.
+SLOTS_PER_POINT_STEP_FIXED = 120.0
 #   streaming regime: bytes of HBM traffic with classical RK4 and one fused pass per stage.
 BYTES_PER_POINT_STEP = 384.0
 # FP64 ALU peak: 148 SMs x 64 DFMA lanes/clk x sm_max_mhz (derived in DESIGN.md; the
@@ -53,6 +56,8 @@ def parse():
     ap.add_argument("--batch", type=int, default=0, help="override the ensemble size (0 = workload default)")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 persistent streaming, 2 resident, 3 generic streaming")
     ap.add_argument("--variant", type=int, default=None, help="resident kernel variant (tuning; default auto)")
+    ap.add_argument("--fixed-background", action="store_true",
+                    help="time the fixed-background variant (A = 1, delta = 0 held fixed; PAPER.md:177 Table II)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -119,7 +124,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_rate(name, N, seconds, rk4_cap=None):
+def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False):
     """Time the oracle as it stands on the host cores on a bounded sample of the workload:
     2 x cores members (or the whole batch if smaller), enough RK4 steps for ~`seconds`."""
     import oracle
@@ -130,7 +135,7 @@ def oracle_rate(name, N, seconds, rk4_cap=None):
     B = min(Bfull, 2 * thr)
     thr = min(thr, B)
     Phi, Pi, _ = inputs.make(name, B=B)
-    ev = oracle.Evolution(Phi, Pi, nthreads=thr)
+    ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=fixed)
     t = time.perf_counter(); ev.step(2); cal = (time.perf_counter() - t) / 2
     n = max(2, int(seconds / max(cal, 1e-9)))
     if rk4_cap:
@@ -159,7 +164,7 @@ def run_reference(args):
     B = min(inputs.CONFIGS[name]["B"], 2 * thr)
     thr = min(thr, B)
     Phi, Pi, _ = inputs.make(name, B=B)
-    ev = oracle.Evolution(Phi, Pi, nthreads=thr)
+    ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=args.fixed_background)
     t = time.perf_counter(); ev.step(2); cal = (time.perf_counter() - t) / 2
     budget = max(1.0, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
     n = max(1, int(budget / max(cal, 1e-9)))
@@ -178,7 +183,7 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic (seeded, paper_1706_07413_b200/inputs.py)",
         "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_sampled": B, "rk4_per_step": n,
-                   "courant": 0.25, "ko_eps": 0.1},
+                   "courant": 0.25, "ko_eps": 0.1, "fixed_background": bool(args.fixed_background)},
         "cpu_baseline": {"value": rate, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -222,7 +227,8 @@ def main():
     Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all[lo:hi])).pin_memory()
     del Phi_all, Pi_all
 
-    ens = binding.Ensemble(N, B, device=dev, path=args.path, resident_variant=args.variant)
+    ens = binding.Ensemble(N, B, device=dev, path=args.path, resident_variant=args.variant,
+                           fixed_background=args.fixed_background)
     path, cluster = ens.path
     Phi_d, Pi_d = Phi_h.to(dev), Pi_h.to(dev)
     ens.set_initial(Phi_d, Pi_d)
@@ -293,18 +299,19 @@ def main():
     per_gpu_rate = value / world
     if path == 2:
         peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
-        ach_tf = per_gpu_rate * SLOTS_PER_POINT_STEP * 2 / 1e12
+        slots = SLOTS_PER_POINT_STEP_FIXED if args.fixed_background else SLOTS_PER_POINT_STEP
+        ach_tf = per_gpu_rate * slots * 2 / 1e12
         roof = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(name) if B == cfg["B"] else None,
+                "frac": ach_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(name) if (B == cfg["B"] and not args.fixed_background) else None,
                 "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
                 "kernel": "k_resident3 (whole RK4 steps on chip; 1 launch per adsc_step)",
                 "peak_src": f"derived: {N_SMS} SMs x {FP64_LANES_PER_SM} DFMA lanes x "
                             f"{peaks['sm_max_mhz']:.0f} MHz x 2 flop (DESIGN.md Roofline)",
-                "algorithmic": f"{SLOTS_PER_POINT_STEP:.0f} FP64-pipe instr per point per RK4 step"}
+                "algorithmic": f"{slots:.0f} FP64-pipe instr per point per RK4 step"}
     else:
         ach = per_gpu_rate * BYTES_PER_POINT_STEP / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(name) if B == cfg["B"] else None,
+                "frac": ach / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(name) if (B == cfg["B"] and not args.fixed_background) else None,
                 "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
                 "kernel": ("k_stream_persist (stage state in shared memory, u^n/accumulator through L2; "
                            "1 cooperative launch per adsc_step)" if path == 1 else
@@ -314,14 +321,14 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
-        cpu, _, _, _ = oracle_rate(name, N, args.cpu_seconds)
+        cpu, _, _, _ = oracle_rate(name, N, args.cpu_seconds, fixed=args.fixed_background)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic (seeded, paper_1706_07413_b200/inputs.py)",
         "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_per_gpu": B, "global_batch": B * world,
-                   "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1,
+                   "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1, "fixed_background": bool(args.fixed_background),
                    "path": {1: "streaming-persistent", 2: "resident", 3: "streaming-generic"}[path],
                    "ctas_per_member": cluster,
                    "parallelism": f"members sharded over {world} GPU(s), no collective",

@@ -69,6 +69,16 @@ extern "C" {
                                           threads, default).  Results do not depend on it beyond
                                           rounding order.                                       */
 
+#define ADSC_OPT_FIXED_BACKGROUND    7  /* 1: evolve on the fixed background A = 1, delta = 0 (the
+                                          paper's second workload, Table II): the
+                                          delta integration, the exponential and the A update are
+                                          compiled out of the stage kernels; adsc_set_initial sets
+                                          A = 1 without solving eq (5); K_A is ignored; no member
+                                          ever collapses; adsc_get_fields returns delta = 0; the
+                                          diagnostics use A = 1 (mass = linear energy, residual =
+                                          max |1 - A^c|).  Set it before adsc_bind (ESTATE
+                                          afterwards).  Default 0.                              */
+
 typedef struct adsc_ctx *adsc_handle;
 
 /* One record per member, filled by adsc_diagnostics (host memory). */

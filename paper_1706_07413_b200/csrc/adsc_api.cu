@@ -86,6 +86,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->pb.dt = courant * c->pb.h;
     c->pb.ko_eps = ko_eps;
     c->pb.thr = 0.0078125;   // 2^-7 (BASELINE.json configs[1])
+    c->pb.fixed_bg = 0;
     c->K_A = 0; c->path_opt = 0; c->steps_per_launch = 0;
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
@@ -148,6 +149,13 @@ int adsc_set_option(adsc_handle h, int key, double value)
         }
         return ADSC_OK;
     }
+    case ADSC_OPT_FIXED_BACKGROUND:
+        if (!(value == 0.0 || value == 1.0)) return fail(h, ADSC_EINVAL, "fixed background: 0 or 1");
+        if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_FIXED_BACKGROUND before adsc_bind");
+        h->pb.fixed_bg = (int)value;
+        resolve_path(h);                 // not every resident configuration has a fixed-background kernel
+        if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
+        return ADSC_OK;
     case ADSC_OPT_STREAM_PPT:
         if (!(value == 2.0 || value == 4.0)) return fail(h, ADSC_EINVAL, "points per thread of the streaming kernel: 2 or 4");
         h->sp_ppt = (int)value;
@@ -213,6 +221,7 @@ static int set_common(adsc_handle h, const double *d_Phi, const double *d_Pi, co
     ADSC_CUDA(launch_pack(h, d_Phi, 0, true), "pack Phi");
     ADSC_CUDA(launch_pack(h, d_Pi, 1, false), "pack Pi");
     if (d_A) ADSC_CUDA(launch_pack(h, d_A, 2, false), "pack A");
+    else if (h->pb.fixed_bg) ADSC_CUDA(launch_fill(h, h->ws.U[2], 1.0), "A = 1");
     else ADSC_CUDA(launch_solve(h, SOLVE_WRITE_A), "constraint solve");
     h->have_state = true;
     h->global_step = 0;
@@ -254,7 +263,7 @@ int adsc_step(adsc_handle h, long long nsteps)
     if (!h) return fail(nullptr, ADSC_EINVAL, "null handle");
     if (!h->bound || !h->have_state) return fail(h, ADSC_ESTATE, "adsc_bind and adsc_set_initial first");
     if (nsteps < 0) return fail(h, ADSC_EINVAL, "nsteps must be >= 0");
-    const int K = h->K_A;
+    const int K = h->pb.fixed_bg ? 0 : h->K_A;
     if (h->path == 2 || h->path == 1) {
         long long left = nsteps;
         while (left > 0) {
@@ -315,7 +324,8 @@ int adsc_get_fields(adsc_handle h, double *d_Phi, double *d_Pi, double *d_A, dou
     }
     if (d_delta) {
         if ((uintptr_t)d_delta & 7u) return fail(h, ADSC_EINVAL, "field pointers must be 8-byte aligned");
-        ADSC_CUDA(launch_solve(h, 0), "delta solve");
+        if (h->pb.fixed_bg) ADSC_CUDA(launch_fill(h, h->ws.dl, 0.0), "delta = 0");
+        else ADSC_CUDA(launch_solve(h, 0), "delta solve");
         ADSC_CUDA(launch_unpack(h, h->ws.dl, d_delta), "unpack delta");
     }
     return ADSC_OK;
@@ -332,7 +342,8 @@ int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A
         double *stage = h->ws.stage[v & 1];
         if (v < 3) ADSC_CUDA(launch_unpack(h, h->ws.U[v], stage), "unpack");
         else {
-            ADSC_CUDA(launch_solve(h, 0), "delta solve");
+            if (h->pb.fixed_bg) ADSC_CUDA(launch_fill(h, h->ws.dl, 0.0), "delta = 0");
+            else ADSC_CUDA(launch_solve(h, 0), "delta solve");
             ADSC_CUDA(launch_unpack(h, h->ws.dl, stage), "unpack delta");
         }
         ADSC_CUDA(cudaMemcpyAsync(dst[v], stage, n, cudaMemcpyDeviceToHost, h->stream), "D2H field");

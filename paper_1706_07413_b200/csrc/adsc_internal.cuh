@@ -40,6 +40,7 @@ struct Tables {
 
 struct Problem {
     int N, NP, B;
+    int fixed_bg;        // PAPER.md:177 (Table II): A and delta held fixed at 1 and 0 -- no scan, no exp, A not evolved
     double h, dt, ko_eps, thr;
 };
 
@@ -102,6 +103,7 @@ namespace adsc {
 cudaError_t launch_tables(adsc_ctx *c);
 cudaError_t launch_pack(adsc_ctx *c, const double *src, int field, bool init_rec);
 cudaError_t launch_unpack(adsc_ctx *c, const double *src_internal, double *dst);
+cudaError_t launch_fill(adsc_ctx *c, double *dst_internal, double value);   // whole [B][NP] array
 // mode bits for launch_solve
 enum { SOLVE_WRITE_A = 1, SOLVE_DIAG = 2, SOLVE_ACTIVE_ONLY = 4 };
 cudaError_t launch_solve(adsc_ctx *c, int mode);              // one CTA per member, or the tiled kernels for long members

@@ -363,11 +363,12 @@ static const ResConfig &cfg_at(int k)
 {
     return k < n_cfgs3 ? g_cfgs3[k] : g_cfgs1[k - n_cfgs3];
 }
-static const void *fn_for(const ResConfig &g, int cl)
+static const void *fn_for(const ResConfig &g, int cl, int fixed_bg)
 {
-    if (cl == 1) return g.fn[0];
-    if (g.any_cl) return g.fn[1];
-    return cl == 2 ? g.fn[1] : cl == 4 ? g.fn[2] : cl == 8 ? g.fn[3] : nullptr;
+    const void *const *fn = fixed_bg ? g.fnf : g.fn;
+    if (cl == 1) return fn[0];
+    if (g.any_cl) return fn[1];
+    return cl == 2 ? fn[1] : cl == 4 ? fn[2] : cl == 8 ? fn[3] : nullptr;
 }
 
 const char *resident_cfg_name(int cfg) { return (cfg >= 0 && cfg < n_cfgs()) ? cfg_at(cfg).name : "none"; }
@@ -383,7 +384,7 @@ bool resident_select(adsc_ctx *c)
         if (n_act % g.seg) continue;
         const int cl = n_act / g.seg;
         if (cl < 1 || cl > 8) continue;
-        if (!fn_for(g, cl)) continue;
+        if (!fn_for(g, cl, c->pb.fixed_bg)) continue;
         if (c->dev_smem_optin > 0 && g.smem > (size_t)c->dev_smem_optin) continue;
         c->res_cfg = k; c->cluster = cl;
         return true;
@@ -394,7 +395,8 @@ bool resident_select(adsc_ctx *c)
 cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last)
 {
     const ResConfig &g = cfg_at(c->res_cfg);
-    const void *fn = fn_for(g, c->cluster);
+    const void *fn = fn_for(g, c->cluster, c->pb.fixed_bg);
+    if (!fn) return cudaErrorInvalidDeviceFunction;      // adsc_step checks this combination before launching
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
     if (e != cudaSuccess) return e;
     ResParams prm;

@@ -40,6 +40,7 @@ struct ResConfig {
     size_t smem;
     bool any_cl;
     const void *fn[4];
+    const void *fnf[4];    // the same for the fixed background A = 1, delta = 0 (nullptr: not compiled)
 };
 
 // generation-3 table (adsc_resident3.cu); the generation-1 table is local to adsc_resident.cu

@@ -105,7 +105,9 @@ __device__ __forceinline__ void st_async_f64x2(uint32_t dst_cluster, double v0, 
                  ::"r"(dst_cluster), "l"(__double_as_longlong(v0)), "l"(__double_as_longlong(v1)), "r"(mbar_cluster) : "memory");
 }
 
-template <int P, int THREADS, bool ACC_REG, int CL>
+// FIXED: the paper's second workload (Table II), A = 1 and delta = 0 held fixed: no f', no scan,
+// no exponential, eq (4) not evolved, no collapse test -- the same stencils, exchanges and RK combine.
+template <int P, int THREADS, bool ACC_REG, int CL, bool FIXED>
 __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resident3(const __grid_constant__ ResParams prm)
 {
     using L = Res3Layout<P, THREADS, ACC_REG, CL>;
@@ -144,7 +146,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
     // sync points: S is double-buffered by the parity of its index, F is single
     const uint32_t mbS0 = smem_u32(smem + L::o_mbar), mbS1 = mbS0 + 8, mbF = mbS0 + 16;
     // transaction bytes this CTA receives from its peers per sync
-    const uint32_t txS = MULTI ? (uint32_t)((rank > 0 ? 48 : 0) + (rank < CL - 1 ? 48 : 0) + (CL - 1) * NW * 16) : 0u;
+    const uint32_t txS = MULTI ? (uint32_t)((rank > 0 ? 48 : 0) + (rank < CL - 1 ? 48 : 0) + (FIXED ? 0 : (CL - 1) * NW * 16)) : 0u;
     const uint32_t txF = MULTI ? (uint32_t)((rank > 0 ? 32 : 0) + (rank < CL - 1 ? 32 : 0)) : 0u;
     if (tid == 0) {
         mbar_init(mbS0, NW); mbar_init(mbS1, NW); mbar_init(mbF, NW);
@@ -211,12 +213,14 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
     // f', s of the new state; publish the state edges and the warp total for sync S with index parity jb.
     auto publish_S = [&](const int jb, const bool with_flag) {
         const uint32_t mb = jb ? mbS1 : mbS0;
+        if constexpr (!FIXED) {
 #pragma unroll
-        for (int p = 0; p < P; ++p) fo[p] = tSC[p * LD + col] * fma(ph[p], ph[p], pi[p] * pi[p]);
-        // top term of the telescoped rule: S_{N-1} = S_N = f_{N-2}/12 (f_N = -f_{N-2}, f_{N-1} = 0)
-        so[P - 1] = fo[P - 1] + (last ? fo[P - 1] * (1.0 / 12.0) : 0.0);
+            for (int p = 0; p < P; ++p) fo[p] = tSC[p * LD + col] * fma(ph[p], ph[p], pi[p] * pi[p]);
+            // top term of the telescoped rule: S_{N-1} = S_N = f_{N-2}/12 (f_N = -f_{N-2}, f_{N-1} = 0)
+            so[P - 1] = fo[P - 1] + (last ? fo[P - 1] * (1.0 / 12.0) : 0.0);
 #pragma unroll
-        for (int p = P - 2; p >= 0; --p) so[p] = so[p + 1] + fo[p];
+            for (int p = P - 2; p >= 0; --p) so[p] = so[p + 1] + fo[p];
+        }
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             xPhi[k * LD + col] = ph[k]; xPi[k * LD + col] = pi[k];
@@ -252,25 +256,30 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 }
             }
         }
-        // a2, warp level: inclusive suffix over the lanes; the warp total (and collapse flag) goes to every CTA.
-        // The shuffle chain (5 dependent steps) is pure latency, so the own-point Kreiss-Oliger sums of the
-        // first NFILL points are written between its steps: one basic block, ptxas interleaves them.
-        double incl = so[0];
+        if constexpr (FIXED) {
 #pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            const double o = __shfl_down_sync(FULL, incl, 1 << k);
-            if (k < NFILL) ko_pt(k);
-            if (lane + (1 << k) < 32) incl += o;
-        }
-        excl = incl - so[0];
-        const double wsum = __shfl_sync(FULL, incl, 0);
-        double flag = 0.0;
-        if (with_flag) flag = __any_sync(FULL, bad) ? 1.0 : 0.0;
-        double2 *slot = wt + jb * NG + gw;
-        if (lane == 0) *slot = make_double2(wsum, flag);
-        if (MULTI) {
-            if (lane < CL && lane != rank)
-                st_async_f64x2(map_rank(smem_u32(slot), lane), wsum, flag, map_rank(mb, lane));
+            for (int k = 0; k < NFILL; ++k) ko_pt(k);
+        } else {
+            // a2, warp level: inclusive suffix over the lanes; the warp total (and collapse flag) goes to every CTA.
+            // The shuffle chain (5 dependent steps) is pure latency, so the own-point Kreiss-Oliger sums of the
+            // first NFILL points are written between its steps: one basic block, ptxas interleaves them.
+            double incl = so[0];
+#pragma unroll
+            for (int k = 0; k < 5; ++k) {
+                const double o = __shfl_down_sync(FULL, incl, 1 << k);
+                if (k < NFILL) ko_pt(k);
+                if (lane + (1 << k) < 32) incl += o;
+            }
+            excl = incl - so[0];
+            const double wsum = __shfl_sync(FULL, incl, 0);
+            double flag = 0.0;
+            if (with_flag) flag = __any_sync(FULL, bad) ? 1.0 : 0.0;
+            double2 *slot = wt + jb * NG + gw;
+            if (lane == 0) *slot = make_double2(wsum, flag);
+            if (MULTI) {
+                if (lane < CL && lane != rank)
+                    st_async_f64x2(map_rank(smem_u32(slot), lane), wsum, flag, map_rank(mb, lane));
+            }
         }
         warp_arrive(mb, txS);
     };
@@ -301,26 +310,6 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 hlP[k] = xPhi[(RX - 3 + k) * LD + col - 1]; hlQ[k] = xPi[(RX - 3 + k) * LD + col - 1];
                 hrP[k] = xPhi[k * LD + col + 1];            hrQ[k] = xPi[k * LD + col + 1];
             }
-            const double scm = tSC[(P - 1) * LD + col - 1], scp = tSC[0 * LD + col + 1];
-            // a2, member level: all f' above this thread's points (predicates are warp- / CTA-uniform)
-            double B0 = excl, B1 = 0.0;
-            {
-                const double2 *wl = wts + rank * NW;
-#pragma unroll
-                for (int w = 1; w < NW; ++w) {
-                    if (w > warp) { if (w & 1) B1 += wl[w].x; else B0 += wl[w].x; }
-                }
-                if (MULTI) {
-#pragma unroll
-                    for (int r = 1; r < CL; ++r) {
-                        if (r > rank) {
-#pragma unroll
-                            for (int w = 0; w < NW; ++w) { if (w & 1) B1 += wts[r * NW + w].x; else B0 += wts[r * NW + w].x; }
-                        }
-                    }
-                }
-            }
-            const double B = B0 + B1;
             // halo part of the Kreiss-Oliger sums
 #pragma unroll
             for (int p = 0; p < P; ++p) {
@@ -330,25 +319,50 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                     if (p + j >= P) { kP[p] = fma(K.kw[j], hrP[p + j - P], kP[p]); kQ[p] = fma(K.kw[j], hrQ[p + j - P], kQ[p]); }
                 }
             }
-            // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f
-            double nd[P];
-            {
-                const double fm = scm * fma(hlP[2], hlP[2], hlQ[2] * hlQ[2]);     // f'_{-1}
-                const double fp = scp * fma(hrP[0], hrP[0], hrQ[0] * hrQ[0]);     // f'_{P}
-                const double top = last ? fo[P - 1] * (1.0 / 12.0) : 0.0;         // as in publish_S
-#pragma unroll
-                for (int p = 0; p < P; ++p) {
-                    const double f_lo = (p == 0) ? fm : fo[p - 1];
-                    const double f_hi = (p == P - 1) ? fp : fo[p + 1];
-                    const double s2 = (p + 2 < P) ? so[p + 2] : ((p + 2 == P) ? top : top - fp);
-                    double loc = K.c25 * f_hi;
-                    loc = fma(K.c12, fo[p], loc);
-                    loc = fma(-K.c1, f_lo, loc);
-                    nd[p] = fma(K.hh, s2 + B, loc);
-                }
-            }
             double E[P];
-            exp3_near<P>(nd, E);
+            if constexpr (FIXED) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) E[p] = 1.0;                   // delta = 0 held fixed
+            } else {
+                const double scm = tSC[(P - 1) * LD + col - 1], scp = tSC[0 * LD + col + 1];
+                // a2, member level: all f' above this thread's points (predicates are warp- / CTA-uniform)
+                double B0 = excl, B1 = 0.0;
+                {
+                    const double2 *wl = wts + rank * NW;
+#pragma unroll
+                    for (int w = 1; w < NW; ++w) {
+                        if (w > warp) { if (w & 1) B1 += wl[w].x; else B0 += wl[w].x; }
+                    }
+                    if (MULTI) {
+#pragma unroll
+                        for (int r = 1; r < CL; ++r) {
+                            if (r > rank) {
+#pragma unroll
+                                for (int w = 0; w < NW; ++w) { if (w & 1) B1 += wts[r * NW + w].x; else B0 += wts[r * NW + w].x; }
+                            }
+                        }
+                    }
+                }
+                const double B = B0 + B1;
+                // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f
+                double nd[P];
+                {
+                    const double fm = scm * fma(hlP[2], hlP[2], hlQ[2] * hlQ[2]);     // f'_{-1}
+                    const double fp = scp * fma(hrP[0], hrP[0], hrQ[0] * hrQ[0]);     // f'_{P}
+                    const double top = last ? fo[P - 1] * (1.0 / 12.0) : 0.0;         // as in publish_S
+#pragma unroll
+                    for (int p = 0; p < P; ++p) {
+                        const double f_lo = (p == 0) ? fm : fo[p - 1];
+                        const double f_hi = (p == P - 1) ? fp : fo[p + 1];
+                        const double s2 = (p + 2 < P) ? so[p + 2] : ((p + 2 == P) ? top : top - fp);
+                        double loc = K.c25 * f_hi;
+                        loc = fma(K.c12, fo[p], loc);
+                        loc = fma(-K.c1, f_lo, loc);
+                        nd[p] = fma(K.hh, s2 + B, loc);
+                    }
+                }
+                exp3_near<P>(nd, E);
+            }
             // a3 fluxes
             double H[P], F[P], kAv[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
 #pragma unroll
@@ -361,7 +375,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 if (p == 2) G2 = G;
                 if (p == P - 1) Gl1 = G;
                 if (p == P - 2) Gl2 = G;
-                kAv[p] = (tSC[p * LD + col] * a[p]) * (G * pi[p]);        // eq (4): -2 sc A G Pi
+                if constexpr (FIXED) kAv[p] = 0.0;                        // A = 1 held fixed
+                else kAv[p] = (tSC[p * LD + col] * a[p]) * (G * pi[p]);   // eq (4): -2 sc A G Pi
             }
             if (first) kAv[0] = 0.0;                                      // A(0,t)=1, eq (8)
             // publish flux edges
@@ -395,7 +410,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
 
             // ---------------------------------------------------------------- between arrive and wait
             // a4/a5 for A (eq 4 needs no neighbour).  Invariant at the start of every step: acc == u^n == state.
-            if (s < 3) {
+            if constexpr (FIXED) {
+                // A is not evolved
+            } else if (s < 3) {
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
                     const int ui = (2 * P + p) * THREADS + tid;
@@ -491,9 +508,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
             if (s == 3) {
                 // a6: collapse test of PAPER.md:85 on A^{n+1}: every warp of the member published its flag
                 int any = 0;
-                const int2 *fl = reinterpret_cast<const int2 *>(wt + jb * NG);
+                if constexpr (!FIXED) {
+                    const int2 *fl = reinterpret_cast<const int2 *>(wt + jb * NG);
 #pragma unroll
-                for (int w = 0; w < NG; ++w) any |= fl[2 * w + 1].y;      // high word of the flag (0.0 or 1.0)
+                    for (int w = 0; w < NG; ++w) any |= fl[2 * w + 1].y;  // high word of the flag (0.0 or 1.0)
+                }
                 n_done = n + 1;
                 if (any && (prm.check_last || n + 1 < prm.nsteps)) collapsed = 1;
             }
@@ -523,14 +542,24 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
 }
 
 // ------------------------------------------------------------------ configuration table
-#define ADSC_RES3_FN(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_>
+#define ADSC_RES3_FN(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false>
+#define ADSC_RES3_FNF(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, true>
+// fn: dynamical A, delta; fnf: fixed background, nullptr where not compiled (tuning variants)
 #define ADSC_RES3_CFG_ALL(P_, T_, ACC_)                                                               \
     { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 8>::bytes, false,       \
       { ADSC_RES3_FN(P_, T_, ACC_, 1), ADSC_RES3_FN(P_, T_, ACC_, 2), ADSC_RES3_FN(P_, T_, ACC_, 4),    \
-        ADSC_RES3_FN(P_, T_, ACC_, 8) } }
+        ADSC_RES3_FN(P_, T_, ACC_, 8) },                                                              \
+      { ADSC_RES3_FNF(P_, T_, ACC_, 1), ADSC_RES3_FNF(P_, T_, ACC_, 2), ADSC_RES3_FNF(P_, T_, ACC_, 4), \
+        ADSC_RES3_FNF(P_, T_, ACC_, 8) } }
 #define ADSC_RES3_CFG_ONE(P_, T_, ACC_)                                                               \
     { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 1>::bytes, false,       \
-      { ADSC_RES3_FN(P_, T_, ACC_, 1), nullptr, nullptr, nullptr } }
+      { ADSC_RES3_FN(P_, T_, ACC_, 1), nullptr, nullptr, nullptr },                                   \
+      { ADSC_RES3_FNF(P_, T_, ACC_, 1), nullptr, nullptr, nullptr } }
+#define ADSC_RES3_CFG_TUNE(P_, T_, ACC_)                                                              \
+    { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 8>::bytes, false,       \
+      { ADSC_RES3_FN(P_, T_, ACC_, 1), ADSC_RES3_FN(P_, T_, ACC_, 2), ADSC_RES3_FN(P_, T_, ACC_, 4),    \
+        ADSC_RES3_FN(P_, T_, ACC_, 8) },                                                              \
+      { nullptr, nullptr, nullptr, nullptr } }
 
 const ResConfig g_cfgs3[] = {
     ADSC_RES3_CFG_ALL(8, 256, true),    // SEG 2048, accumulators in registers: N-1 = 2048, 4096, 8192, 16384
@@ -538,8 +567,8 @@ const ResConfig g_cfgs3[] = {
     ADSC_RES3_CFG_ONE(4, 128, false),   // SEG 512
     ADSC_RES3_CFG_ONE(4, 64, false),    // SEG 256
     ADSC_RES3_CFG_ONE(4, 32, false),    // SEG 128
-    ADSC_RES3_CFG_ALL(8, 128, true),    // SEG 1024, two CTAs per SM (tuning)
-    ADSC_RES3_CFG_ALL(4, 512, true),    // SEG 2048, 16 warps (tuning)
+    ADSC_RES3_CFG_TUNE(8, 128, true),   // SEG 1024, two CTAs per SM (tuning)
+    ADSC_RES3_CFG_TUNE(4, 512, true),   // SEG 2048, 16 warps (tuning)
 };
 const int n_cfgs3 = sizeof(g_cfgs3) / sizeof(g_cfgs3[0]);
 

@@ -96,6 +96,20 @@ __global__ void k_unpack(Problem pb, const double *__restrict__ src, double *__r
     if (i < pb.N) dst[(size_t)b * pb.N + i] = src[(size_t)b * pb.NP + i];
 }
 
+__global__ void k_fill(size_t n, double *__restrict__ dst, double value)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = value;
+}
+
+cudaError_t launch_fill(adsc_ctx *c, double *dst_internal, double value)
+{
+    const size_t n = (size_t)c->pb.B * c->pb.NP;
+    k_fill<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, dst_internal, value);
+    c->launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_unpack(adsc_ctx *c, const double *src_internal, double *dst)
 {
     dim3 grid((c->pb.N + 255) / 256, c->pb.B);

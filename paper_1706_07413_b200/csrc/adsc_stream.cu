@@ -92,8 +92,8 @@ __device__ __forceinline__ Flux flux_phys(const Problem &pb, const Tables &tb, c
                                           const double *Pi, const double *A, const double *dl,
                                           const double *carry, int m)
 {
-    const double delta = dl[m] + carry[m / GEN_TILE];
-    const double AE = A[m] * exp(-delta);
+    // fixed background: delta = 0 is not integrated, e^{-delta} = 1
+    const double AE = pb.fixed_bg ? A[m] : A[m] * exp(-(dl[m] + carry[m / GEN_TILE]));
     Flux r;
     r.G = AE * Phi[m];
     r.H = AE * Pi[m];
@@ -190,7 +190,7 @@ k_stream_rhs(Problem pb, Tables tb, StageIO io, const double *__restrict__ gdl,
             k[1] = 3.0 * d4c * (sG[s - 2] - 8.0 * sG[s - 1] + 8.0 * sG[s + 1] - sG[s + 2]) + qPi;
         else
             k[1] = tb.C[i] * (d4c * (sF[s - 2] - 8.0 * sF[s - 1] + 8.0 * sF[s + 1] - sF[s + 2])) + qPi;
-        k[2] = -2.0 * tb.sc[i] * a_own[q] * sG[s] * pi_own[q];
+        k[2] = pb.fixed_bg ? 0.0 : -2.0 * tb.sc[i] * a_own[q] * sG[s] * pi_own[q];
         if (i == 0) { k[0] = 0.0; k[2] = 0.0; }
         if (i == N - 1) { k[0] = 0.0; k[1] = 0.0; k[2] = 0.0; }
 #pragma unroll
@@ -204,7 +204,7 @@ k_stream_rhs(Problem pb, Tables tb, StageIO io, const double *__restrict__ gdl,
                 io.out[v][g] = base_un + a_next * k[v];
             } else {
                 io.out[v][g] = accn;
-                if (v == 2 && !(accn >= pb.thr)) bad = 1;
+                if (v == 2 && !pb.fixed_bg && !(accn >= pb.thr)) bad = 1;
             }
         }
     }
@@ -221,12 +221,15 @@ cudaError_t launch_stream_step(adsc_ctx *c)
     for (int s = 0; s < 4; ++s) {
         double *const *in = (s == 0) ? w.U : (s == 2 ? w.Ub : w.Ua);
         double *const *out = (s == 0 || s == 2) ? w.Ua : (s == 1 ? w.Ub : w.U);
-        k_stream_I<<<grid, GEN_THREADS, 0, c->stream>>>(c->pb, c->tb, in[0], in[1], w.dl, w.tot, w.rec, nt);
-        k_stream_carry<<<c->pb.B, GEN_THREADS, 0, c->stream>>>(w.tot, w.carry, w.rec, nt);
+        if (!c->pb.fixed_bg) {
+            k_stream_I<<<grid, GEN_THREADS, 0, c->stream>>>(c->pb, c->tb, in[0], in[1], w.dl, w.tot, w.rec, nt);
+            k_stream_carry<<<c->pb.B, GEN_THREADS, 0, c->stream>>>(w.tot, w.carry, w.rec, nt);
+            c->launches += 2;
+        }
         StageIO io;
         for (int v = 0; v < 3; ++v) { io.in[v] = in[v]; io.un[v] = w.U[v]; io.acc[v] = w.ACC[v]; io.out[v] = out[v]; }
         k_stream_rhs<<<grid, GEN_THREADS, 0, c->stream>>>(c->pb, c->tb, io, w.dl, w.carry, w.rec, nt, s);
-        c->launches += 3;
+        c->launches += 1;
     }
     return cudaGetLastError();
 }

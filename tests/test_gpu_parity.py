@@ -302,3 +302,48 @@ def test_error_codes(env):
     assert lib.adsc_destroy(None) == 0
     with pytest.raises(binding.AdscError):
         binding.Ensemble(2 ** 20 + 1, 1, path=2)     # does not fit on chip
+
+
+# ------------------------------------------------- f1: fixed background A = 1, delta = 0 (Table II)
+
+@pytest.mark.parametrize("name,B,N,path,nsteps", [
+    ("cfg5", 6, 2049, 2, 1000),      # resident, one CTA per member
+    ("cfg2", 3, 4097, 2, 1000),      # resident, cluster of 2
+    ("cfg3", 2, 8193, 2, 400),       # resident, cluster of 4
+    ("cfg5", 3, 1025, 2, 500),       # resident, small configuration (P8xT128)
+    ("cfg2", 2, 65537, 1, 60),       # persistent streaming: the paper's Table II size, N = 64K
+    ("cfg2", 2, 65537, 3, 60),       # generic streaming kernels
+    ("cfg5", 3, 1027, 1, 300),       # persistent streaming, N-1 = 2 mod 4
+])
+def test_fixed_background_matches_oracle(env, name, B, N, path, nsteps):
+    """the same stage kernels with the scan, the exponential and the A update compiled out.
+    Strong data (amplitudes that would collapse with a dynamical metric): the evolution is linear."""
+    Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
+    x = env["inputs"].grid(N)
+    Phi = Phi + 3.0 * np.sin(2 * x)[None, :] * np.cos(x)[None, :] ** 2
+    Phi[:, 0] = 0; Phi[:, -1] = 0
+    Pi = Pi * 20.0
+    ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=path, fixed_background=True)
+    assert ens.path[0] == path
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 8), fixed_background=True).step(nsteps)
+    scale = max(1.0, np.abs(ev.Pi).max())
+    for k, ref in (("Phi", ev.Phi), ("Pi", ev.Pi)):
+        assert np.isfinite(f[k]).all()
+        assert np.max(np.abs(f[k] - ref)) <= TOL * scale, (k, np.max(np.abs(f[k] - ref)))
+    assert (f["A"] == 1).all() and (f["delta"] == 0).all()
+    assert (f["Phi"][:, 0] == 0).all() and (f["Phi"][:, -1] == 0).all() and (f["Pi"][:, -1] == 0).all()
+    assert (d["steps_done"] == nsteps).all() and (d["collapsed"] == 0).all()
+    od = ev.diagnostics()
+    assert np.max(np.abs(d["mass"] - od["mass"]) / np.abs(od["mass"])) <= 1e-11
+    assert (d["min_A"] == 1).all()
+
+
+def test_fixed_background_option_order(env):
+    binding = env["binding"]
+    lib = binding.load_library()
+    ens = binding.Ensemble(1025, 1)
+    assert lib.adsc_set_option(ens.h, binding.ADSC_OPT_FIXED_BACKGROUND, 1.0) == binding.ADSC_ESTATE   # after bind
+    h = lib.adsc_create(1025, 1, 0.25, 0.1)
+    assert lib.adsc_set_option(h, binding.ADSC_OPT_FIXED_BACKGROUND, 2.0) == binding.ADSC_EINVAL
+    assert lib.adsc_set_option(h, binding.ADSC_OPT_FIXED_BACKGROUND, 1.0) == 0
+    lib.adsc_destroy(h)
