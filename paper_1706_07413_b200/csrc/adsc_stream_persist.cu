@@ -14,16 +14,15 @@
 //             E = e^{-delta}, fluxes G, H, F, D4 and Kreiss-Oliger stencils, RK combine, in-place
 //             write of the new stage state, running sum of the NEW state's f' for the next stage.
 // The discrete algorithm is DESIGN.md section 1; nothing here is shared with oracle/.
-#include "adsc_internal.cuh"
+#include "adsc_stream_persist.cuh"
 #include "adsc_exp.cuh"
 
 namespace adsc {
 
 constexpr int SP_TILE = 1024;                      // points per tile = threads x contiguous points per thread
 constexpr int SP_TILES = 7;                        // tiles per chunk
-constexpr int SP_CAP = SP_TILE * SP_TILES;         // 7168 points per CTA
+static_assert(SP_CAP == SP_TILE * SP_TILES, "7168 points per CTA");
 constexpr int SP_HAL = 4;                          // lower halo slots of the chunk arrays (3 used)
-constexpr int SP_MBOX = 24;                        // doubles per chunk mailbox
 
 // Shared-memory index map: thread t touches P t + q (P = 2 or 4), a stride of P doubles; one padding
 // double per 16 makes those accesses conflict-free (16 consecutive lanes, 16 distinct 8-byte banks).
@@ -44,46 +43,6 @@ struct SPLayout {
     static constexpr int n_doubles = o_eT + 6 * (SP_TILES + 1);
     static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
 };
-
-struct SPConsts {
-    double d4c, kw[4], hh, c25, c12, c1, inv12h2, c_org, a_next[4], b_w[4], thr;
-};
-
-struct SPParams {
-    Problem pb;
-    Tables tb;
-    double *U[3];
-    double *ACC[3];
-    MemberRec *rec;
-    double *mbox;                    // [groups][2][G][SP_MBOX]
-    unsigned long long *counter;     // [groups], zeroed before the launch
-    long long nsteps;
-    int check_last;
-    int G, groups, Lc;               // chunks per member, concurrent members, points per chunk
-    SPConsts k;
-};
-
-// ---- grid barrier over the G CTAs of one member (all co-resident: cooperative launch)
-__device__ __forceinline__ void group_barrier(unsigned long long *cnt, unsigned long long target)
-{
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(cnt, 1ULL);
-        unsigned long long v;
-        do {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(cnt) : "memory");
-        } while (v < target);
-    }
-    __syncthreads();
-}
-
-__device__ __forceinline__ double ld_cg(const double *p)
-{
-    double v;
-    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
-    return v;
-}
 
 // Sum over the CTA (result valid in every thread).  sw: 40 doubles.
 template <int T>
@@ -525,14 +484,16 @@ bool stream_persist_select(adsc_ctx *c)
     const int gmax = (N + SP_TILE - 1) / SP_TILE;
     if (G > gmax) G = gmax;
     if (G < gmin) G = gmin;
-    int Lc = ((N + G - 1) / G + 3) / 4 * 4;
+    if (c->pb.fixed_bg && c->sp_ppt == 8) c->sp_ppt = 4;     // the 8-point kernel has no fixed-background build
+    if (c->sp_ppt != 2 && c->sp_ppt != 4 && c->sp_ppt != 8) c->sp_ppt = 8;
+    const int al = (c->sp_ppt == 8) ? 8 : 4;                 // chunks start on a thread boundary
+    int Lc = ((N + G - 1) / G + al - 1) / al * al;
     G = (N + Lc - 1) / Lc;
     if (Lc > SP_CAP || (G > 1 && N - (G - 1) * Lc < 8)) return false;
     int groups = sms / G;
     if (groups > c->pb.B) groups = c->pb.B;
     if (groups < 1 || (size_t)groups * G > SP_MAX_CTAS) return false;
     c->sp_G = G; c->sp_Lc = Lc; c->sp_groups = groups; c->sp_ok = true;
-    if (c->sp_ppt != 2 && c->sp_ppt != 4) c->sp_ppt = 4;
     return true;
 }
 
@@ -562,6 +523,11 @@ cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
         k.a_next[0] = 0.5 * dt; k.a_next[1] = 0.5 * dt; k.a_next[2] = dt; k.a_next[3] = 0.0;
         k.b_w[0] = dt / 6.0; k.b_w[1] = dt / 3.0; k.b_w[2] = dt / 3.0; k.b_w[3] = dt / 6.0;
         k.thr = c->pb.thr;
+    }
+    if (c->sp_ppt == 8) {
+        e = launch_stream_persist8(c, prm);
+        c->launches++;
+        return e;
     }
     void *args[] = { (void *)&prm };
     e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)(c->sp_G * c->sp_groups)), dim3((unsigned)threads), args,
