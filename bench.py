@@ -58,6 +58,9 @@ def parse():
     ap.add_argument("--variant", type=int, default=None, help="resident kernel variant (tuning; default auto)")
     ap.add_argument("--fixed-background", action="store_true",
                     help="time the fixed-background variant (A = 1, delta = 0 held fixed; PAPER.md:177 Table II)")
+    ap.add_argument("--masked-fraction", type=float, default=0.0,
+                    help="force this fraction of the members to collapse during warm-up (Pi x 1000): shows that masked "
+                         "members cost nothing; the metric then counts the members still active (SURVEY.md 8(d))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -223,6 +226,10 @@ def main():
     # Rank r evolves members [r*B, (r+1)*B) of the (tiled) seeded ensemble: no exchange step.
     lo, hi = shard.member_range(rank, world, B * world)
     Phi_all, Pi_all, _ = inputs.make(name, B=hi)
+    if args.masked_fraction > 0.0:
+        bidx = np.arange(lo, hi)
+        forced = np.floor((bidx + 1) * args.masked_fraction) > np.floor(bidx * args.masked_fraction)
+        Pi_all[lo:hi][forced] *= 1.0e3            # collapses within the first warm-up steps
     Phi_h = torch.from_numpy(np.ascontiguousarray(Phi_all[lo:hi])).pin_memory()
     Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all[lo:hi])).pin_memory()
     del Phi_all, Pi_all
@@ -263,7 +270,13 @@ def main():
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    updates = float(B) * world * N * rk4 * K
+    n_active = float((d["collapsed"] == 0).sum())
+    if dist is not None:
+        t = torch.tensor([n_active], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        n_active = float(t.item())
+    # members still active x N x RK4 steps; without forced collapses every member is active
+    updates = (n_active if args.masked_fraction > 0.0 else float(B) * world) * N * rk4 * K
     value = updates / (ms * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers: H2D of Phi, Pi + step + D2H of the fields
@@ -286,7 +299,7 @@ def main():
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
-    e2e_value = float(B) * world * N * rk4 * Ke / e2e_s
+    e2e_value = (updates / K) * Ke / e2e_s
     h2d = 2 * B * N * 8
     d2h = 3 * B * N * 8 + B * binding.DIAG_DTYPE.itemsize
 
@@ -333,7 +346,7 @@ def main():
                    "ctas_per_member": cluster,
                    "parallelism": f"members sharded over {world} GPU(s), no collective",
                    "l2": "flushed between timed iterations (256 MiB fill)",
-                   "active_fraction": active_frac},
+                   "active_fraction": active_frac, "masked_fraction_forced": args.masked_fraction},
         "roofline": roof,
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
