@@ -13,7 +13,8 @@ Workloads (BASELINE.json configs; recipe in DESIGN.md "Input recipe"):
   cfg5  N=2049  B=16384  Gaussian Pi, sigma~U[0.2,0.5], eps~U[0.05,0.5]
   tcollapse N=1025 B=64  Gaussian Pi, sigma=1/16, eps~U[30,60] (test only)
 The paper's own initial data are mode sums with Phi(x,0)=0 (PAPER.md:89-93,
-111); no public dataset is involved, these seeded ensembles stand in.
+111); no public dataset is involved, these seeded ensembles stand in.  qp_family()
+generates the paper's families themselves (eq (13)) for the t_c(eps) driver.
 """
 from __future__ import annotations
 
@@ -66,6 +67,36 @@ def eigenmode(j: int, x: np.ndarray):
     e = d * c ** 3 * F
     de = d * (-3.0 * c ** 2 * s * F + c ** 3 * dF * 2.0 * s * c)
     return e, de
+
+
+def eigenmode_jacobi(j: int, x: np.ndarray) -> np.ndarray:
+    """e_j through the Jacobi polynomial, 2F1(-j, 3+j; 3/2; sin^2 x) = j!/(3/2)_j P_j^(1/2,3/2)(cos 2x): the
+    three-term recurrence stays accurate for the high modes of the paper's mode-sum data (the terminating
+    series of eigenmode() loses digits to cancellation beyond j ~ 10)."""
+    from scipy.special import eval_jacobi, gammaln
+    d = math.sqrt(16.0 * (j + 1) * (j + 2) / math.pi)
+    norm = math.exp(gammaln(j + 1.0) + gammaln(1.5) - gammaln(j + 1.5))
+    return d * np.cos(x) ** 3 * norm * eval_jacobi(j, 0.5, 1.5, np.cos(2.0 * x))
+
+
+def qp_family(N: int, eps, mu: float, kd: int, kmax: int | None = None):
+    """The paper's approximately quasi-periodic families (eq (13)):
+    mode amplitudes A_k = eps exp(-mu |k - k_d|), initial data with Phi(x,0) = 0 (Fig. 2 caption,
+    PAPER.md:111).  Reading R23: phi = sum_k A_k e_k sin(omega_k t), so Pi(x,0) = sum_k A_k omega_k e_k(x).
+    eps scalar or [B] (one member per amplitude); modes k = 0..kmax, kmax defaults to where the tail is
+    below 1e-17 of the peak.  Returns (Phi, Pi, A_k[B][kmax+1])."""
+    eps = np.atleast_1d(np.asarray(eps, dtype=np.float64))
+    if kmax is None:
+        kmax = kd + int(math.ceil(39.2 / mu))
+    x = grid(N)
+    k = np.arange(kmax + 1)
+    shape = np.exp(-mu * np.abs(k - kd))
+    prof = np.zeros(N)
+    for j in k:
+        prof += shape[j] * omega(int(j)) * eigenmode_jacobi(int(j), x)
+    Pi = eps[:, None] * prof[None, :]
+    Pi[:, -1] = 0.0
+    return np.zeros_like(Pi), Pi, eps[:, None] * shape[None, :]
 
 
 def omega(j: int) -> float:

@@ -348,3 +348,24 @@ def test_fixed_background_option_order(env):
     assert lib.adsc_set_option(h, binding.ADSC_OPT_FIXED_BACKGROUND, 2.0) == binding.ADSC_EINVAL
     assert lib.adsc_set_option(h, binding.ADSC_OPT_FIXED_BACKGROUND, 1.0) == 0
     lib.adsc_destroy(h)
+
+
+# ------------------------------------------------- f4: t_c(eps) driver on the paper's families
+
+def test_tc_sweep_driver_matches_oracle(env):
+    """the driver (paper_1706_07413_b200/tc_sweep.py) on the family k_d = 3, mu = 1 of eq (13),
+    threshold 0.01: flags identical to the oracle's, collapse times within one step, and t_c
+    decreasing with the amplitude."""
+    from paper_1706_07413_b200 import tc_sweep
+    eps = np.array([0.03, 0.05, 0.08])
+    N, tmax = 1025, 6.0
+    r = tc_sweep.sweep(eps, 1.0, 3, N=N, tmax=tmax, threshold=0.01)
+    Phi, Pi, _ = env["inputs"].qp_family(N, eps, 1.0, 3)
+    ev = env["oracle"].Evolution(Phi, Pi, thr=0.01, nthreads=3)
+    ev.step(int(np.ceil(tmax / ev.dt)))
+    od = ev.diagnostics()
+    assert (r["collapsed"] == od["collapsed"]).all() and r["collapsed"].tolist() == [0, 1, 1]
+    for b in (1, 2):
+        assert abs(r["t_collapse"][b] - od["t_collapse"][b]) <= ev.dt * (1 + 1e-12)
+    assert r["t_collapse"][2] < r["t_collapse"][1]
+    assert np.isnan(r["t_collapse"][0]) and r["mass_loss"][0] < 1e-8

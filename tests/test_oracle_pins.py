@@ -432,3 +432,24 @@ def test_F3_dynamical_evolution_tends_to_fixed_background_as_amplitude_vanishes(
         fix = oracle.Evolution(eps * Phi0, np.zeros(N), fixed_background=True).step(400)
         d.append(np.abs(dyn.Phi[0] - fix.Phi[0]).max() / eps)
     assert d[0] < 1e-2 and 50 < d[0] / d[1] < 200, d
+
+
+# ------------------------------------------------- f4: the paper's data families (input generator pins)
+
+def test_F4_qp_family_generator_has_the_prescribed_spectrum():
+    # PAPER.md:93-101 eq (13): A_k = eps exp(-mu |k - k_d|), Phi(x,0) = 0; reading R23:
+    # Pi(x,0) = sum_k A_k omega_k e_k.  Orthonormality of the e_k under tan^2 x dx (R19) must give the
+    # spectrum back; the Jacobi form of e_j must agree with the terminating series where that one is accurate.
+    N = 2049
+    x = inputs.grid(N); tb = oracle.tables(N)
+    for j in range(6):
+        e, _ = inputs.eigenmode(j, x)
+        assert np.abs(inputs.eigenmode_jacobi(j, x) - e).max() < 5e-13
+    eps = np.array([0.01, 0.04])
+    Phi, Pi, Ak = inputs.qp_family(N, eps, 1.75, 5)
+    assert (Phi == 0).all() and (Pi[:, -1] == 0).all() and Ak.shape[0] == 2
+    assert np.allclose(Ak[1] / Ak[0], 4.0) and np.argmax(Ak[0]) == 5 and abs(Ak[0][5] - 0.01) < 1e-18
+    assert abs(Ak[0][7] / Ak[0][5] - np.exp(-3.5)) < 1e-15
+    for k in range(12):
+        proj = (tb["w"][:-1] * tb["T"][:-1] * Pi[0][:-1] * inputs.eigenmode_jacobi(k, x)[:-1]).sum()
+        assert abs(proj / inputs.omega(k) - Ak[0][k]) < 1e-12 * Ak[0][5], k
