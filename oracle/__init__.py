@@ -178,5 +178,21 @@ class Evolution:
         return d
 
 
+def eigenmode(N: int, j: int):
+    """AdS4 normal mode e_j and e_j' on the grid (Jacobi recurrence in long double)."""
+    e, de = np.zeros(N), np.zeros(N)
+    assert lib().oracle_eigenmode(C.c_int(N), C.c_int(j), _p(e), _p(de)) == 0
+    return e, de
+
+
+def mode_energies(Phi, Pi, J: int):
+    """E_j = Pi_j^2 + Phi_j^2/omega_j^2, j < J, per member (reading R24); also the projections."""
+    Phi, Pi = (_f64(np.atleast_2d(a)) for a in (Phi, Pi))
+    B, N = Phi.shape
+    E = np.zeros((B, J)); proj = np.zeros((B, J, 2))
+    assert lib().oracle_mode_energies(C.c_int(N), C.c_int(B), C.c_int(J), _p(Phi), _p(Pi), _p(E), _p(proj)) == 0
+    return E, proj
+
+
 def max_threads() -> int:
     return int(lib().oracle_max_threads())

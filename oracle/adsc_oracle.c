@@ -472,6 +472,83 @@ int oracle_evolve_fixed(int N, int B, double courant, double ko_eps,
     return evolve(N, B, courant, ko_eps, 0.0, 0, 1, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
 }
 
+/* ---------------------------------------------------- normal-mode projection (f3)
+ * "At any given time, the current numerical solution can be decomposed into a
+ * spectrum of normal modes".  AdS4 modes (R19): e_j = d_j cos^3 x
+ * 2F1(-j, 3+j; 3/2; sin^2 x), d_j = sqrt(16(j+1)(j+2)/pi), omega_j = 3+2j,
+ * orthonormal under tan^2 x dx; their derivatives are orthogonal with norm
+ * omega_j^2.  2F1(-j,3+j;3/2;z) = j!/(3/2)_j P_j^{(1/2,3/2)}(1-2z), evaluated by
+ * the three-term Jacobi recurrence in long double.  Reading R24: with
+ * Pi_j = int Pi e_j tan^2 x dx and Phi_j = int Phi e_j' tan^2 x dx (composite
+ * Simpson, integrand := 0 at i = N-1 as in R15) the mode energy is
+ * E_j = Pi_j^2 + Phi_j^2 / omega_j^2, so that sum_j E_j -> M in the linear limit. */
+static long double jacobi(int n, long double a, long double b, long double y)
+{
+    if (n < 0) return 0.0L;
+    long double p0 = 1.0L;
+    if (n == 0) return p0;
+    long double p1 = (a + 1.0L) + (a + b + 2.0L) * (y - 1.0L) / 2.0L;
+    for (int m = 2; m <= n; ++m) {
+        long double c = 2.0L * m + a + b;
+        long double a1 = 2.0L * m * (m + a + b) * (c - 2.0L);
+        long double a2 = (c - 1.0L) * (c * (c - 2.0L) * y + a * a - b * b);
+        long double a3 = 2.0L * (m + a - 1.0L) * (m + b - 1.0L) * c;
+        long double p2 = (a2 * p1 - a3 * p0) / a1;
+        p0 = p1; p1 = p2;
+    }
+    return p1;
+}
+
+static void eigenmode(int j, long double x, long double *e, long double *de)
+{
+    const long double pi = 2.0L * PI_2L;
+    long double d = sqrtl(16.0L * (j + 1) * (j + 2) / pi);
+    long double nrm = 1.0L;                      /* j! / (3/2)_j */
+    for (int m = 1; m <= j; ++m) nrm *= (long double)m / ((long double)m + 0.5L);
+    long double s = sinl(x), c = cosl(x), y = cosl(2.0L * x);
+    long double P = jacobi(j, 0.5L, 1.5L, y);
+    long double dP = 0.5L * (j + 3.0L) * jacobi(j - 1, 1.5L, 2.5L, y);      /* dP/dy */
+    *e = d * nrm * c * c * c * P;
+    *de = d * nrm * (-3.0L * c * c * s * P + c * c * c * dP * (-2.0L * sinl(2.0L * x)));
+}
+
+/* e_j and e_j' on the grid (for the pins). */
+int oracle_eigenmode(int N, int j, double *e, double *de)
+{
+    for (int i = 0; i < N; ++i) {
+        long double x = (i == N - 1) ? PI_2L : PI_2L * (long double)i / (long double)(N - 1);
+        long double a, b;
+        eigenmode(j, x, &a, &b);
+        e[i] = (double)a; de[i] = (double)b;
+    }
+    return 0;
+}
+
+/* out[b][j] = E_j, proj[b][2j] = Pi_j, proj[b][2j+1] = Phi_j (proj may be NULL). */
+int oracle_mode_energies(int N, int B, int J, const double *Phi, const double *Pi, double *out, double *proj)
+{
+    tables tb; if (tables_init(&tb, N)) return -1;
+    for (int j = 0; j < J; ++j) {
+        long double om = 3.0L + 2.0L * j;
+        for (int b = 0; b < B; ++b) {
+            const double *ph = Phi + (size_t)b * N, *pi = Pi + (size_t)b * N;
+            long double sp = 0.0L, sf = 0.0L;
+            for (int i = 0; i < N - 1; ++i) {
+                long double x = PI_2L * (long double)i / (long double)(N - 1);
+                long double e, de;
+                eigenmode(j, x, &e, &de);
+                long double wt = (long double)tb.w[i] * (long double)tb.T[i];
+                sp += wt * (long double)pi[i] * e;
+                sf += wt * (long double)ph[i] * de;
+            }
+            out[(size_t)b * J + j] = (double)(sp * sp + sf * sf / (om * om));
+            if (proj) { proj[((size_t)b * J + j) * 2] = (double)sp; proj[((size_t)b * J + j) * 2 + 1] = (double)sf; }
+        }
+    }
+    tables_free(&tb);
+    return 0;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

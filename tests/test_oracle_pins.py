@@ -453,3 +453,36 @@ def test_F4_qp_family_generator_has_the_prescribed_spectrum():
     for k in range(12):
         proj = (tb["w"][:-1] * tb["T"][:-1] * Pi[0][:-1] * inputs.eigenmode_jacobi(k, x)[:-1]).sum()
         assert abs(proj / inputs.omega(k) - Ak[0][k]) < 1e-12 * Ak[0][5], k
+
+
+# ------------------------------------------------- f3: normal-mode projection
+
+def test_F5_mode_projection_orthonormality_parseval_and_spectrum():
+    # (i) the oracle's Jacobi-recurrence modes agree with the terminating hypergeometric series of the input
+    #     generator where that one is accurate (independent routes to the same e_j, e_j');
+    # (ii) Pi = e_k gives E_j = delta_jk, Phi = e_k' gives E_j = omega_k^2 delta_jk (R19; Simpson, 4th order);
+    # (iii) Parseval in the linear limit: two-mode data, sum_j E_j = M(A = 1) (R15, R24);
+    # (iv) the family of eq (13): sqrt(E_k)/omega_k = A_k.
+    N, J = 1025, 8
+    x = inputs.grid(N); tb = oracle.tables(N)
+    for j in (0, 2, 5):
+        e, de = inputs.eigenmode(j, x)
+        eo, deo = oracle.eigenmode(N, j)
+        assert np.abs(e - eo).max() < 1e-12 and np.abs(de - deo).max() < 1e-11
+    for k in (0, 3):
+        e, de = oracle.eigenmode(N, k)
+        E, _ = oracle.mode_energies(np.zeros(N), e, J)
+        ref = np.zeros(J); ref[k] = 1.0
+        assert np.abs(E[0] - ref).max() < 1e-8, E
+        E, _ = oracle.mode_energies(de, np.zeros(N), J)
+        ref[k] = (3.0 + 2 * k) ** 2
+        assert np.abs(E[0] - ref).max() < 1e-6, E
+    Phi, Pi = inputs.two_mode(N, [0.05], [0.6], [1.1])
+    E, proj = oracle.mode_energies(Phi, Pi, J)
+    M = (tb["w"][:-1] * tb["T"][:-1] * (Phi[0][:-1] ** 2 + Pi[0][:-1] ** 2)).sum()
+    assert abs(E[0].sum() / M - 1.0) < 1e-8 and E[0][2:].max() < 1e-12 * M
+    assert abs(E[0][1] / E[0][0] - 0.6) < 1e-8                  # the energy ratio of R20
+    Phi, Pi, Ak = inputs.qp_family(N, [0.02], 1.0, 3)
+    E, _ = oracle.mode_energies(Phi, Pi, J)
+    om = 3.0 + 2.0 * np.arange(J)
+    assert np.abs(np.sqrt(E[0]) / om - Ak[0][:J]).max() < 1e-9 * Ak[0][3]
