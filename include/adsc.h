@@ -153,6 +153,14 @@ int adsc_get_fields(adsc_handle h, double *d_Phi, double *d_Pi, double *d_A, dou
 int adsc_set_initial_host(adsc_handle h, const double *h_Phi, const double *h_Pi);
 int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta);
 
+/* Normal-mode spectrum of the current state ("the current numerical solution can be
+ * decomposed into a spectrum of normal modes").  For the AdS4 modes e_j (R19),
+ * j < J <= 32: Pi_j = int Pi e_j tan^2 x dx, Phi_j = int Phi e_j' tan^2 x dx (composite Simpson, integrand 0
+ * at x = pi/2), E_j = Pi_j^2 + Phi_j^2 / omega_j^2, omega_j = 3 + 2j (R24).  host_out: HOST array
+ * [batch][J], row-major, owned by the caller.  One kernel launch plus one small D2H copy; synchronises the
+ * stream.  EINVAL for J outside 1..32 or a NULL pointer, ESTATE before adsc_set_initial. */
+int adsc_mode_energies(adsc_handle h, int J, double *host_out);
+
 /* Number of kernels this handle has launched since adsc_bind (for gpu_launches). */
 long long adsc_launch_count(adsc_handle h);
 

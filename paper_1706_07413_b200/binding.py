@@ -60,6 +60,7 @@ _SIGS = {
     "adsc_get_fields": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_set_initial_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_get_fields_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "adsc_mode_energies": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
     "adsc_launch_count": (C.c_longlong, [C.c_void_p]),
     "adsc_path": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
     "adsc_last_error": (C.c_char_p, [C.c_void_p]),
@@ -145,6 +146,10 @@ def adsc_set_initial_host(h, h_Phi, h_Pi):
 
 def adsc_get_fields_host(h, h_Phi, h_Pi, h_A, h_delta):
     _check(h, load_library().adsc_get_fields_host(h, h_Phi, h_Pi, h_A, h_delta))
+
+
+def adsc_mode_energies(h, J, host_out_ptr):
+    _check(h, load_library().adsc_mode_energies(h, int(J), host_out_ptr))
 
 
 def adsc_launch_count(h):
@@ -257,6 +262,13 @@ class Ensemble:
         out = np.zeros(self.batch, dtype=DIAG_DTYPE)
         with self.torch.cuda.device(self.device):
             adsc_diagnostics(self.h, out.ctypes.data)
+        return out
+
+    def mode_energies(self, J):
+        """[batch][J] normal-mode energies E_j of the current state (adsc_mode_energies)."""
+        out = np.zeros((self.batch, int(J)), dtype=np.float64)
+        with self.torch.cuda.device(self.device):
+            adsc_mode_energies(self.h, J, out.ctypes.data)
         return out
 
     def get_fields(self, delta=True):

@@ -352,6 +352,20 @@ int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A
     return ADSC_OK;
 }
 
+int adsc_mode_energies(adsc_handle h, int J, double *host_out)
+{
+    if (!h) return fail(nullptr, ADSC_EINVAL, "null handle");
+    if (!h->bound || !h->have_state) return fail(h, ADSC_ESTATE, "adsc_bind and adsc_set_initial first");
+    if (!host_out) return fail(h, ADSC_EINVAL, "null output");
+    if (J < 1 || J > 32 || J > h->pb.NP) return fail(h, ADSC_EINVAL, "J must be in 1..32 (and <= N)");
+    double *d_out = h->ws.Ac;                    // scratch: [B][NP] doubles, enough for [B][J]
+    ADSC_CUDA(launch_mode_energies(h, J, d_out), "mode projection kernel");
+    ADSC_CUDA(cudaMemcpyAsync(host_out, d_out, (size_t)h->pb.B * J * sizeof(double), cudaMemcpyDeviceToHost, h->stream),
+              "D2H mode energies");
+    ADSC_CUDA(cudaStreamSynchronize(h->stream), "stream synchronize");
+    return ADSC_OK;
+}
+
 long long adsc_launch_count(adsc_handle h) { return h ? h->launches : 0; }
 
 int adsc_path(adsc_handle h, int *cluster)

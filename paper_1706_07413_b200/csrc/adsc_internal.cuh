@@ -110,6 +110,7 @@ cudaError_t launch_solve(adsc_ctx *c, int mode);              // one CTA per mem
 cudaError_t launch_solve_tiled(adsc_ctx *c, int mode);        // adsc_solve_tiled.cu (streaming layouts only)
 constexpr int SOLVE_TILED_MIN_N = 32768;                      // members at least this long use the tiled solve
 cudaError_t launch_finalize(adsc_ctx *c, int inc_steps);
+cudaError_t launch_mode_energies(adsc_ctx *c, int J, double *d_out);   // adsc_modes.cu; d_out [B][J]
 cudaError_t launch_stream_step(adsc_ctx *c);                 // one RK4 step, generic streaming kernels
 bool stream_persist_select(adsc_ctx *c);                     // fills c->sp_* (needs c->dev_sms)
 cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last);   // persistent streaming kernel

@@ -1,0 +1,126 @@
+// adsc_modes.cu — normal-mode projection diagnostic: "the current numerical solution can
+// be decomposed into a spectrum of normal modes".  For the AdS4 modes (R19)
+//   e_j = d_j cos^3 x 2F1(-j, 3+j; 3/2; sin^2 x),  d_j = sqrt(16 (j+1)(j+2)/pi),  omega_j = 3 + 2j,
+// and j < J:  Pi_j = int Pi e_j tan^2 x dx,  Phi_j = int Phi e_j' tan^2 x dx  (composite Simpson, integrand := 0
+// at x = pi/2, as for the mass, R15),  E_j = Pi_j^2 + Phi_j^2 / omega_j^2  (R24; sum_j E_j -> M in the linear limit).
+// It is a [J x N] . [N x B] contraction whose left factor is never stored: every thread rebuilds the J mode
+// values of its grid points with the three-term Jacobi recurrence, 2F1(-j,3+j;3/2;z) = j!/(3/2)_j P_j^{(1/2,3/2)}(1-2z)
+// and dP_j^{(a,b)}/dy = (j+a+b+1)/2 P_{j-1}^{(a+1,b+1)}.  One CTA per member; off the per-stage path.
+#include <cmath>
+
+#include "adsc_internal.cuh"
+
+namespace adsc {
+
+constexpr int MODES_MAX = 32;
+constexpr int MODES_THREADS = 256;
+
+struct ModeCoef {
+    // P_n = (r1[n] y + r2[n]) P_{n-1} - r3[n] P_{n-2} for the families (1/2,3/2) [0] and (3/2,5/2) [1]
+    double r1[2][MODES_MAX], r2[2][MODES_MAX], r3[2][MODES_MAX];
+    double p1c[2][2];            // P_1 = p1c[.][0] + p1c[.][1] (y - 1)
+    double dn[MODES_MAX];        // d_j j!/(3/2)_j
+    double dq[MODES_MAX];        // (j + 3)/2: dP_j/dy = dq[j] Q_{j-1}
+    double iom2[MODES_MAX];      // 1/omega_j^2
+};
+
+__global__ void __launch_bounds__(MODES_THREADS)
+k_mode_energies(Problem pb, Tables tb, const double *__restrict__ gPhi, const double *__restrict__ gPi,
+                const __grid_constant__ ModeCoef mc, int J, double *__restrict__ out)
+{
+    __shared__ double red[2][MODES_THREADS / 32];
+    const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = pb.N;
+    const double *Phi = gPhi + (size_t)b * pb.NP, *Pi = gPi + (size_t)b * pb.NP;
+    double sp[MODES_MAX], sf[MODES_MAX];
+#pragma unroll
+    for (int j = 0; j < MODES_MAX; ++j) { sp[j] = 0.0; sf[j] = 0.0; }
+    for (int i = tid; i < N - 1; i += MODES_THREADS) {        // the integrand is 0 at i = N-1
+        double s, c;
+        sincospi((double)i / (2.0 * (double)(N - 1)), &s, &c);
+        const double y = c * c - s * s, s2 = 2.0 * s * c, c2 = c * c, c3 = c2 * c;
+        const double wt = tb.w[i] * tb.T[i];
+        const double wp = wt * Pi[i], wf = wt * Phi[i];
+        double p0 = 1.0, p1 = mc.p1c[0][0] + mc.p1c[0][1] * (y - 1.0);      // P_{j-1}, P_j of (1/2, 3/2) at j = 1
+        double q0 = 0.0, q1 = 1.0;                                          // Q_{j-2}, Q_{j-1} of (3/2, 5/2) at j = 1
+#pragma unroll
+        for (int j = 0; j < MODES_MAX; ++j) {
+            if (j < J) {
+                double Pj, Qjm1;
+                if (j == 0) { Pj = 1.0; Qjm1 = 0.0; }
+                else if (j == 1) { Pj = p1; Qjm1 = 1.0; }
+                else {
+                    const double p2 = (mc.r1[0][j] * y + mc.r2[0][j]) * p1 - mc.r3[0][j] * p0;
+                    p0 = p1; p1 = p2; Pj = p2;
+                    double q2;                                              // Q_{j-1}: index n = j-1 of family 1
+                    if (j == 2) q2 = mc.p1c[1][0] + mc.p1c[1][1] * (y - 1.0);
+                    else q2 = (mc.r1[1][j - 1] * y + mc.r2[1][j - 1]) * q1 - mc.r3[1][j - 1] * q0;
+                    q0 = q1; q1 = q2; Qjm1 = q2;
+                }
+                const double e = mc.dn[j] * c3 * Pj;
+                const double de = mc.dn[j] * (-3.0 * c2 * s * Pj - 2.0 * s2 * c3 * mc.dq[j] * Qjm1);
+                sp[j] = fma(wp, e, sp[j]);
+                sf[j] = fma(wf, de, sf[j]);
+            }
+        }
+    }
+    // CTA reduction, mode by mode (fixed order: deterministic)
+#pragma unroll 1
+    for (int j = 0; j < J; ++j) {
+        double a = 0.0, f = 0.0;
+#pragma unroll
+        for (int k = 0; k < MODES_MAX; ++k) if (k == j) { a = sp[k]; f = sf[k]; }
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) {
+            a += __shfl_down_sync(0xffffffffu, a, d);
+            f += __shfl_down_sync(0xffffffffu, f, d);
+        }
+        __syncthreads();
+        if (lane == 0) { red[0][warp] = a; red[1][warp] = f; }
+        __syncthreads();
+        if (tid == 0) {
+            double A = 0.0, F = 0.0;
+            for (int w = 0; w < MODES_THREADS / 32; ++w) { A += red[0][w]; F += red[1][w]; }
+            out[(size_t)b * J + j] = A * A + F * F * mc.iom2[j];
+        }
+    }
+}
+
+// coefficients of the Jacobi recurrence 2n(n+a+b)(2n+a+b-2) P_n =
+//   (2n+a+b-1)[(2n+a+b)(2n+a+b-2) y + a^2 - b^2] P_{n-1} - 2(n+a-1)(n+b-1)(2n+a+b) P_{n-2}
+static void fill_coef(ModeCoef &mc)
+{
+    const double ab[2][2] = { { 0.5, 1.5 }, { 1.5, 2.5 } };
+    for (int f = 0; f < 2; ++f) {
+        const double a = ab[f][0], b = ab[f][1];
+        mc.p1c[f][0] = a + 1.0; mc.p1c[f][1] = 0.5 * (a + b + 2.0);
+        for (int n = 0; n < MODES_MAX; ++n) {
+            mc.r1[f][n] = mc.r2[f][n] = mc.r3[f][n] = 0.0;
+            if (n < 2) continue;
+            const double c = 2.0 * n + a + b;
+            const double a1 = 2.0 * n * (n + a + b) * (c - 2.0);
+            mc.r1[f][n] = (c - 1.0) * c * (c - 2.0) / a1;
+            mc.r2[f][n] = (c - 1.0) * (a * a - b * b) / a1;
+            mc.r3[f][n] = 2.0 * (n + a - 1.0) * (n + b - 1.0) * c / a1;
+        }
+    }
+    double nrm = 1.0;
+    for (int j = 0; j < MODES_MAX; ++j) {
+        if (j >= 1) nrm *= (double)j / ((double)j + 0.5);
+        mc.dn[j] = std::sqrt(16.0 * (j + 1.0) * (j + 2.0) / 3.14159265358979323846264338327950288) * nrm;
+        mc.dq[j] = 0.5 * (j + 3.0);
+        const double om = 3.0 + 2.0 * j;
+        mc.iom2[j] = 1.0 / (om * om);
+    }
+}
+
+cudaError_t launch_mode_energies(adsc_ctx *c, int J, double *d_out)
+{
+    ModeCoef mc;
+    fill_coef(mc);
+    k_mode_energies<<<c->pb.B, MODES_THREADS, 0, c->stream>>>(c->pb, c->tb, c->ws.U[0], c->ws.U[1], mc, J, d_out);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace adsc

@@ -369,3 +369,29 @@ def test_tc_sweep_driver_matches_oracle(env):
         assert abs(r["t_collapse"][b] - od["t_collapse"][b]) <= ev.dt * (1 + 1e-12)
     assert r["t_collapse"][2] < r["t_collapse"][1]
     assert np.isnan(r["t_collapse"][0]) and r["mass_loss"][0] < 1e-8
+
+
+# ------------------------------------------------- f3: normal-mode projection diagnostic
+
+@pytest.mark.parametrize("name,B,N,J,nsteps", [("cfg3", 6, 2049, 8, 300), ("cfg2", 3, 4097, 16, 100),
+                                                 ("cfg5", 2, 1025, 32, 0), ("cfg4", 1, 66699, 12, 10)])
+def test_mode_energies_match_oracle(env, name, B, N, J, nsteps):
+    """E_j of the evolved state against the oracle's projection of the
+    oracle-evolved state; for the two-mode data the spectrum stays in modes 0 and 1 at leading order."""
+    Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
+    torch, binding = env["torch"], env["binding"]
+    ens = binding.Ensemble(N, B)
+    ens.set_initial(torch.from_numpy(Phi).cuda(), torch.from_numpy(Pi).cuda())
+    if nsteps:
+        ens.step(nsteps)
+    E = ens.mode_energies(J)
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 8)).step(nsteps)
+    Eo, _ = env["oracle"].mode_energies(ev.Phi, ev.Pi, J)
+    scale = Eo.max(axis=1, keepdims=True)
+    assert np.isfinite(E).all()
+    assert np.max(np.abs(E - Eo) / scale) <= 1e-11, np.max(np.abs(E - Eo) / scale)
+    if name == "cfg3":
+        assert (E[:, 2:].max(axis=1) < 1e-2 * E[:, :2].sum(axis=1)).all()
+    lib = binding.load_library()
+    assert lib.adsc_mode_energies(ens.h, 0, E.ctypes.data) == binding.ADSC_EINVAL
+    assert lib.adsc_mode_energies(ens.h, 33, E.ctypes.data) == binding.ADSC_EINVAL
