@@ -130,10 +130,13 @@ class Evolution:
     """A batch evolved by the oracle: state in numpy, stepped in place."""
 
     def __init__(self, Phi, Pi, courant: float = 0.25, ko_eps: float = 0.1,
-                 thr: float = 2.0 ** -7, K_A: int = 0, nthreads: int = 1, fixed_background: bool = False):
+                 thr: float = 2.0 ** -7, K_A: int = 0, nthreads: int = 1, fixed_background: bool = False,
+                 rk_order: int = 4):
         s = set_initial(Phi, Pi)
         self.Phi, self.Pi, self.A = s["Phi"], s["Pi"], s["A"]
         self.fixed_background = bool(fixed_background)
+        self.rk_order = int(rk_order)
+        assert not (self.fixed_background and self.rk_order != 4)
         if self.fixed_background:          # PAPER.md:177: A and delta held fixed at 1 and 0
             self.A = np.ones_like(self.Phi)
         self.B, self.N = self.Phi.shape
@@ -150,6 +153,16 @@ class Evolution:
             r = lib().oracle_evolve_fixed(
                 C.c_int(self.N), C.c_int(self.B), C.c_double(self.courant), C.c_double(self.ko_eps),
                 C.c_longlong(nsteps), _p(self.Phi), _p(self.Pi), _p(self.A),
+                self.steps_done.ctypes.data_as(C.POINTER(C.c_longlong)),
+                self.collapsed.ctypes.data_as(C.POINTER(C.c_int)), _p(self.t_collapse),
+                C.c_int(self.nthreads))
+            assert r == 0
+            return self
+        if self.rk_order != 4:
+            r = lib().oracle_evolve_rk(
+                C.c_int(self.N), C.c_int(self.B), C.c_double(self.courant), C.c_double(self.ko_eps),
+                C.c_double(self.thr), C.c_int(self.K_A), C.c_int(self.rk_order), C.c_longlong(nsteps),
+                _p(self.Phi), _p(self.Pi), _p(self.A),
                 self.steps_done.ctypes.data_as(C.POINTER(C.c_longlong)),
                 self.collapsed.ctypes.data_as(C.POINTER(C.c_int)), _p(self.t_collapse),
                 C.c_int(self.nthreads))

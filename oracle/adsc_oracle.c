@@ -211,6 +211,7 @@ typedef struct {
     tables tb;
     double ko_eps, dt;
     int fixed_bg;      /* A = 1, delta = 0 held fixed */
+    int rk_order;      /* 4 (classical RK4, R12), 3 (Heun's third-order rule) or 2 (explicit midpoint): R25 */
     rhs_ws ws;
     double *k[3];      /* current stage slope of (Phi, Pi, A)   */
     double *us[3];     /* stage state u*                         */
@@ -223,6 +224,7 @@ static int stepper_init(stepper *st, int N, double courant, double ko_eps)
     memset(st, 0, sizeof(*st));
     if (tables_init(&st->tb, N)) return -1;
     st->ko_eps = ko_eps;
+    st->rk_order = 4;
     st->dt = courant * st->tb.h;
     double **all[] = { &st->ws.delta, &st->ws.f, &st->ws.G, &st->ws.H, &st->ws.F,
                        &st->k[0], &st->k[1], &st->k[2], &st->us[0], &st->us[1], &st->us[2],
@@ -242,32 +244,40 @@ static void stepper_free(stepper *st)
     free(st->scratch);
 }
 
-/* One classical RK4 step (reading R12; "fourth order accurate Runge-Kutta",
- * PAPER.md:57) of u=(Phi,Pi,A): u2=u+dt/2 k1, u3=u+dt/2 k2, u4=u+dt k3,
- * u^{n+1} = u + dt/6 (k1+2k2+2k3+k4). */
+/* One Runge-Kutta step of u=(Phi,Pi,A).  "second, third, and fourth order accurate Runge-Kutta"
+ * (PAPER.md:57); the tableaux are not printed.  Reading R12: classical RK4, u2=u+dt/2 k1, u3=u+dt/2 k2,
+ * u4=u+dt k3, u^{n+1} = u + dt/6 (k1+2k2+2k3+k4).  Reading R25: third order =
+ * Heun's rule, u2=u+dt/3 k1, u3=u+2dt/3 k2, u^{n+1} = u + dt/4 (k1 + 3 k3); second order = explicit
+ * midpoint, u2=u+dt/2 k1, u^{n+1} = u + dt k2.  In all three every stage state is u^n plus a multiple of
+ * the PREVIOUS slope only, which is the form written out below. */
 static void rk4_step(stepper *st, double *Phi, double *Pi, double *A)
 {
     const int N = st->tb.N;
     const double dt = st->dt;
     double *u[3] = { Phi, Pi, A };
-    static const double a_next[4] = { 0.5, 0.5, 1.0, 0.0 };
-    static const double b_w[4] = { 1.0, 2.0, 2.0, 1.0 };
+    static const double a4[4] = { 0.5, 0.5, 1.0, 0.0 }, b4[4] = { 1.0, 2.0, 2.0, 1.0 };     /* x dt/6 */
+    static const double a3[3] = { 1.0 / 3.0, 2.0 / 3.0, 0.0 }, b3[3] = { 0.25, 0.0, 0.75 };
+    static const double a2[2] = { 0.5, 0.0 }, b2[2] = { 0.0, 1.0 };
+    const int ns = st->rk_order;
+    const double *a_next = (ns == 4) ? a4 : (ns == 3) ? a3 : a2;
+    const double *b_w = (ns == 4) ? b4 : (ns == 3) ? b3 : b2;
+    const double fin = (ns == 4) ? dt / 6.0 : dt;      /* the RK4 arithmetic is unchanged: u + (dt/6)(k1+2k2+2k3+k4) */
     for (int v = 0; v < 3; ++v) {
         memcpy(st->us[v], u[v], N * sizeof(double));
         memset(st->acc[v], 0, N * sizeof(double));
     }
-    for (int s = 0; s < 4; ++s) {
+    for (int s = 0; s < ns; ++s) {
         rhs(&st->tb, st->ko_eps, st->fixed_bg, st->us[0], st->us[1], st->us[2],
             st->k[0], st->k[1], st->k[2], &st->ws);
         for (int v = 0; v < 3; ++v)
             for (int i = 0; i < N; ++i) {
                 st->acc[v][i] += b_w[s] * st->k[v][i];
-                if (s < 3) st->us[v][i] = u[v][i] + a_next[s] * dt * st->k[v][i];
+                if (s < ns - 1) st->us[v][i] = u[v][i] + a_next[s] * dt * st->k[v][i];
             }
     }
     for (int v = 0; v < 3; ++v)
         for (int i = 0; i < N; ++i)
-            u[v][i] = u[v][i] + (dt / 6.0) * st->acc[v][i];
+            u[v][i] = u[v][i] + fin * st->acc[v][i];
 }
 
 /* min A and its first index; NaN-ignoring like fmin.  The collapse predicate
@@ -413,7 +423,7 @@ int oracle_diagnostics(int N, int B, const double *Phi, const double *Pi, const 
  * steps_done / collapsed / t_collapse are in-out per-member arrays (a fresh
  * run passes zeros / zeros / NaN).  nthreads>1 runs members in parallel
  * (members are independent; the scans stay serial inside a member). */
-static int evolve(int N, int B, double courant, double ko_eps, double thr, int K_A, int fixed_bg,
+static int evolve(int N, int B, double courant, double ko_eps, double thr, int K_A, int fixed_bg, int rk_order,
                   long long nsteps, double *Phi, double *Pi, double *A,
                   long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
 {
@@ -425,7 +435,7 @@ static int evolve(int N, int B, double courant, double ko_eps, double thr, int K
     {
         stepper st;
         int ok = (stepper_init(&st, N, courant, ko_eps) == 0);
-        st.fixed_bg = fixed_bg;
+        st.fixed_bg = fixed_bg; st.rk_order = rk_order;
         if (!ok) {
 #ifdef _OPENMP
 #pragma omp atomic write
@@ -460,7 +470,7 @@ int oracle_evolve(int N, int B, double courant, double ko_eps, double thr, int K
                   long long nsteps, double *Phi, double *Pi, double *A,
                   long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
 {
-    return evolve(N, B, courant, ko_eps, thr, K_A, 0, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
+    return evolve(N, B, courant, ko_eps, thr, K_A, 0, 4, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
 }
 
 /* Evolution on the fixed background A = 1, delta = 0 (Table II): A is passed
@@ -469,7 +479,7 @@ int oracle_evolve_fixed(int N, int B, double courant, double ko_eps,
                         long long nsteps, double *Phi, double *Pi, double *A,
                         long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
 {
-    return evolve(N, B, courant, ko_eps, 0.0, 0, 1, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
+    return evolve(N, B, courant, ko_eps, 0.0, 0, 1, 4, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
 }
 
 /* ---------------------------------------------------- normal-mode projection (f3)
@@ -547,6 +557,15 @@ int oracle_mode_energies(int N, int B, int J, const double *Phi, const double *P
     }
     tables_free(&tb);
     return 0;
+}
+
+/* The same evolution with the second- or third-order Runge-Kutta rule of reading R25 (rk_order 2, 3; 4 = RK4). */
+int oracle_evolve_rk(int N, int B, double courant, double ko_eps, double thr, int K_A, int rk_order,
+                     long long nsteps, double *Phi, double *Pi, double *A,
+                     long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
+{
+    if (rk_order < 2 || rk_order > 4) return -1;
+    return evolve(N, B, courant, ko_eps, thr, K_A, 0, rk_order, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
 }
 
 int oracle_max_threads(void)

@@ -486,3 +486,28 @@ def test_F5_mode_projection_orthonormality_parseval_and_spectrum():
     E, _ = oracle.mode_energies(Phi, Pi, J)
     om = 3.0 + 2.0 * np.arange(J)
     assert np.abs(np.sqrt(E[0]) / om - Ak[0][:J]).max() < 1e-9 * Ak[0][3]
+
+
+# ------------------------------------------------- f2: second- and third-order Runge-Kutta
+
+def test_F6_rk_orders_of_accuracy():
+    # "second, third, and fourth order accurate Runge-Kutta"; reading R25: Heun's third-order
+    # rule and the explicit midpoint rule.  At FIXED grid the error against a reference with a much smaller
+    # time step is the time-discretisation error: halving dt must divide it by 2^order.
+    N, T = 129, 0.6
+    x = inputs.grid(N)
+    e1, de1 = inputs.eigenmode(1, x)
+    Phi0 = 0.3 * de1; Phi0[0] = Phi0[-1] = 0.0
+    Pi0 = inputs.gaussian_Pi(N, 1.0, 0.25)[0]
+    h = (np.pi / 2) / (N - 1)
+    def run(order, lam):
+        n = int(round(T / (lam * h)))
+        ev = oracle.Evolution(Phi0, Pi0, courant=T / (n * h), ko_eps=0.0, rk_order=order).step(n)
+        return np.concatenate([ev.Phi[0], ev.Pi[0], ev.A[0]])
+    ref = run(4, 0.0125)
+    for order, lo, hi in ((2, 3.5, 4.6), (3, 7.0, 9.2), (4, 14.0, 18.5)):
+        errs = [np.abs(run(order, lam) - ref).max() for lam in (0.4, 0.2, 0.1)]
+        r1, r2 = errs[0] / errs[1], errs[1] / errs[2]
+        assert lo < r1 < hi and lo < r2 < hi, (order, errs, r1, r2)
+    # the three rules are genuinely different programs: at the same dt their results differ by far more than rounding
+    assert np.abs(run(3, 0.2) - run(4, 0.2)).max() > 1e-8
