@@ -58,6 +58,9 @@ def parse():
     ap.add_argument("--variant", type=int, default=None, help="resident kernel variant (tuning; default auto)")
     ap.add_argument("--fixed-background", action="store_true",
                     help="time the fixed-background variant (A = 1, delta = 0 held fixed; PAPER.md:177 Table II)")
+    ap.add_argument("--rk-order", type=int, default=4, choices=[2, 3, 4],
+                    help="Runge-Kutta order (PAPER.md:57; 3 and 2 run on the streaming paths); the metric then counts "
+                         "grid-point steps of that rule and the algorithmic cost scales with the stage count")
     ap.add_argument("--masked-fraction", type=float, default=0.0,
                     help="force this fraction of the members to collapse during warm-up (Pi x 1000): shows that masked "
                          "members cost nothing; the metric then counts the members still active (SURVEY.md 8(d))")
@@ -127,7 +130,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False):
+def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False, rk_order=4):
     """Time the oracle as it stands on the host cores on a bounded sample of the workload:
     2 x cores members (or the whole batch if smaller), enough RK4 steps for ~`seconds`."""
     import oracle
@@ -138,7 +141,7 @@ def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False):
     B = min(Bfull, 2 * thr)
     thr = min(thr, B)
     Phi, Pi, _ = inputs.make(name, B=B)
-    ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=fixed)
+    ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=fixed, rk_order=rk_order)
     t = time.perf_counter(); ev.step(2); cal = (time.perf_counter() - t) / 2
     n = max(2, int(seconds / max(cal, 1e-9)))
     if rk4_cap:
@@ -167,7 +170,7 @@ def run_reference(args):
     B = min(inputs.CONFIGS[name]["B"], 2 * thr)
     thr = min(thr, B)
     Phi, Pi, _ = inputs.make(name, B=B)
-    ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=args.fixed_background)
+    ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=args.fixed_background, rk_order=args.rk_order)
     t = time.perf_counter(); ev.step(2); cal = (time.perf_counter() - t) / 2
     budget = max(1.0, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
     n = max(1, int(budget / max(cal, 1e-9)))
@@ -235,7 +238,7 @@ def main():
     del Phi_all, Pi_all
 
     ens = binding.Ensemble(N, B, device=dev, path=args.path, resident_variant=args.variant,
-                           fixed_background=args.fixed_background)
+                           fixed_background=args.fixed_background, rk_order=(args.rk_order if args.rk_order != 4 else None))
     path, cluster = ens.path
     Phi_d, Pi_d = Phi_h.to(dev), Pi_h.to(dev)
     ens.set_initial(Phi_d, Pi_d)
@@ -312,7 +315,7 @@ def main():
     per_gpu_rate = value / world
     if path == 2:
         peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
-        slots = SLOTS_PER_POINT_STEP_FIXED if args.fixed_background else SLOTS_PER_POINT_STEP
+        slots = (SLOTS_PER_POINT_STEP_FIXED if args.fixed_background else SLOTS_PER_POINT_STEP) * args.rk_order / 4.0
         ach_tf = per_gpu_rate * slots * 2 / 1e12
         roof = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                 "frac": ach_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(name) if (B == cfg["B"] and not args.fixed_background) else None,
@@ -322,7 +325,9 @@ def main():
                             f"{peaks['sm_max_mhz']:.0f} MHz x 2 flop (DESIGN.md Roofline)",
                 "algorithmic": f"{slots:.0f} FP64-pipe instr per point per RK4 step"}
     else:
-        ach = per_gpu_rate * BYTES_PER_POINT_STEP / 1e9
+        # streaming bytes per step: first and last stage 72 B, every middle stage 120 B
+        bytes_step = 72.0 * 2 + 120.0 * (args.rk_order - 2)
+        ach = per_gpu_rate * bytes_step / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": ach / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(name) if (B == cfg["B"] and not args.fixed_background) else None,
                 "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
@@ -330,18 +335,18 @@ def main():
                            "1 cooperative launch per adsc_step)" if path == 1 else
                            "k_stream_rhs (+ k_stream_I, k_stream_carry: 3 launches per RK stage)"),
                 "peak_src": f"{peaks['src']} copy bandwidth (MEASURED_PEAKS.json)",
-                "algorithmic": f"{BYTES_PER_POINT_STEP:.0f} B per point per RK4 step"}
+                "algorithmic": f"{bytes_step:.0f} B per point per step"}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
-        cpu, _, _, _ = oracle_rate(name, N, args.cpu_seconds, fixed=args.fixed_background)
+        cpu, _, _, _ = oracle_rate(name, N, args.cpu_seconds, fixed=args.fixed_background, rk_order=args.rk_order)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic (seeded, paper_1706_07413_b200/inputs.py)",
         "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_per_gpu": B, "global_batch": B * world,
-                   "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1, "fixed_background": bool(args.fixed_background),
+                   "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1, "fixed_background": bool(args.fixed_background), "rk_order": args.rk_order,
                    "path": {1: "streaming-persistent", 2: "resident", 3: "streaming-generic"}[path],
                    "ctas_per_member": cluster,
                    "parallelism": f"members sharded over {world} GPU(s), no collective",

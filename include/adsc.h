@@ -81,6 +81,12 @@ extern "C" {
                                           max |1 - A^c|).  Set it before adsc_bind (ESTATE
                                           afterwards).  Default 0.                              */
 
+#define ADSC_OPT_RK_ORDER            8  /* 4 (default): classical RK4; 3: Heun's third-order rule; 2:
+                                          explicit midpoint ("second, third, and fourth order accurate
+                                          Runge-Kutta"; tableaux are readings R12, R25).
+                                          Orders 2 and 3 run on the streaming paths (the resident
+                                          kernel is RK4 only).  Set it before adsc_bind.           */
+
 typedef struct adsc_ctx *adsc_handle;
 
 /* One record per member, filled by adsc_diagnostics (host memory). */

@@ -23,6 +23,7 @@ ADSC_OPT_STEPS_PER_LAUNCH = 4
 ADSC_OPT_RESIDENT_VARIANT = 5
 ADSC_OPT_STREAM_PPT = 6
 ADSC_OPT_FIXED_BACKGROUND = 7
+ADSC_OPT_RK_ORDER = 8
 PATH_AUTO, PATH_STREAM, PATH_RESIDENT = 0, 1, 2
 
 
@@ -169,7 +170,7 @@ class Ensemble:
 
     def __init__(self, N, batch, courant=0.25, ko_eps=0.1, device="cuda:0", stream=None,
                  path=PATH_AUTO, threshold=None, a_resolve_period=None, steps_per_launch=None,
-                 resident_variant=None, stream_ppt=None, fixed_background=False):
+                 resident_variant=None, stream_ppt=None, fixed_background=False, rk_order=None):
         import torch
         load_library()
         if not torch.cuda.is_available():
@@ -181,6 +182,8 @@ class Ensemble:
         try:
             if fixed_background:
                 adsc_set_option(self.h, ADSC_OPT_FIXED_BACKGROUND, 1)
+            if rk_order is not None:
+                adsc_set_option(self.h, ADSC_OPT_RK_ORDER, rk_order)
             if path != PATH_AUTO:
                 adsc_set_option(self.h, ADSC_OPT_PATH, path)
             if threshold is not None:

@@ -44,7 +44,7 @@ static void compute_layout(adsc_ctx *c)
 
 static void resolve_path(adsc_ctx *c)
 {
-    const bool can_res = resident_select(c);
+    const bool can_res = (c->rk_order == 4) && resident_select(c);
     if (c->path_opt == 1 || c->path_opt == 3) c->path = c->path_opt;
     else if (c->path_opt == 2) c->path = can_res ? 2 : 0;
     else c->path = can_res ? 2 : 1;
@@ -87,6 +87,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->pb.ko_eps = ko_eps;
     c->pb.thr = 0.0078125;   // 2^-7 (BASELINE.json configs[1])
     c->pb.fixed_bg = 0;
+    c->rk_order = 4;
     c->K_A = 0; c->path_opt = 0; c->steps_per_launch = 0;
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
@@ -154,6 +155,13 @@ int adsc_set_option(adsc_handle h, int key, double value)
         if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_FIXED_BACKGROUND before adsc_bind");
         h->pb.fixed_bg = (int)value;
         resolve_path(h);                 // not every resident configuration has a fixed-background kernel
+        if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
+        return ADSC_OK;
+    case ADSC_OPT_RK_ORDER:
+        if (!(value == 2.0 || value == 3.0 || value == 4.0)) return fail(h, ADSC_EINVAL, "Runge-Kutta order: 2, 3 or 4");
+        if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_RK_ORDER before adsc_bind");
+        h->rk_order = (int)value;
+        resolve_path(h);                 // the resident kernel is RK4 only: other orders take a streaming path
         if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
         return ADSC_OK;
     case ADSC_OPT_STREAM_PPT:

@@ -93,11 +93,25 @@ struct adsc_ctx {
     int dev_smem_optin;
     bool sp_ok;              // persistent streaming kernel usable (decided at adsc_bind)
     int sp_G, sp_groups, sp_Lc;   // chunks per member, concurrent members, points per chunk
+    int rk_order;            // 4 (classical RK4, default), 3 (Heun's third-order rule) or 2 (explicit midpoint): R12, R25
     int sp_ppt;              // points per thread of the persistent streaming kernel: 2 (512 threads) or 4 (256)
     std::string err;
 };
 
 namespace adsc {
+
+// Runge-Kutta rules in the form every kernel uses: u_{s+1} = u^n + a_next[s] k_s, u^{n+1} = u^n + sum_s b_w[s] k_s
+// (weights already multiplied by dt).  PAPER.md:57; R12 (classical RK4), R25 (Heun 3, explicit midpoint).
+inline void rk_tableau(int order, double dt, double a_next[4], double b_w[4])
+{
+    for (int s = 0; s < 4; ++s) { a_next[s] = 0.0; b_w[s] = 0.0; }
+    if (order == 2) { a_next[0] = 0.5 * dt; b_w[1] = dt; }
+    else if (order == 3) { a_next[0] = dt / 3.0; a_next[1] = 2.0 * dt / 3.0; b_w[0] = 0.25 * dt; b_w[2] = 0.75 * dt; }
+    else {
+        a_next[0] = 0.5 * dt; a_next[1] = 0.5 * dt; a_next[2] = dt;
+        b_w[0] = dt / 6.0; b_w[1] = dt / 3.0; b_w[2] = dt / 3.0; b_w[3] = dt / 6.0;
+    }
+}
 
 // ---- launchers implemented in the .cu files (all asynchronous on ctx->stream) -----------
 cudaError_t launch_tables(adsc_ctx *c);

@@ -134,7 +134,8 @@ struct StageIO {
 // a3-a6.  Grid (ntiles, B).
 __global__ void __launch_bounds__(GEN_THREADS)
 k_stream_rhs(Problem pb, Tables tb, StageIO io, const double *__restrict__ gdl,
-             const double *__restrict__ gcarry, MemberRec *rec, int ntiles, int stage)
+             const double *__restrict__ gcarry, MemberRec *rec, int ntiles, int stage, int last_stage,
+             double a_next, double b_w)
 {
     __shared__ double sG[GEN_TILE + 2 * HAL], sH[GEN_TILE + 2 * HAL], sF[GEN_TILE + 2 * HAL];
     const int b = blockIdx.y, tile = blockIdx.x, tid = threadIdx.x;
@@ -168,8 +169,6 @@ k_stream_rhs(Problem pb, Tables tb, StageIO io, const double *__restrict__ gdl,
     __syncthreads();
 
     const double d4c = 1.0 / (12.0 * pb.h), koc = pb.ko_eps / (64.0 * pb.h);
-    const double a_next = (stage == 2) ? pb.dt : 0.5 * pb.dt;
-    const double b_w = (stage == 0 || stage == 3) ? pb.dt / 6.0 : pb.dt / 3.0;
     int bad = 0;
 #pragma unroll
     for (int q = 0; q < PPT; ++q) {
@@ -199,7 +198,7 @@ k_stream_rhs(Problem pb, Tables tb, StageIO io, const double *__restrict__ gdl,
             const double base_un = io.un[v][g];
             const double accv = (stage == 0) ? base_un : io.acc[v][g];
             const double accn = accv + b_w * k[v];
-            if (stage < 3) {
+            if (stage < last_stage) {
                 io.acc[v][g] = accn;
                 io.out[v][g] = base_un + a_next * k[v];
             } else {
@@ -208,7 +207,7 @@ k_stream_rhs(Problem pb, Tables tb, StageIO io, const double *__restrict__ gdl,
             }
         }
     }
-    if (stage == 3) {
+    if (stage == last_stage) {
         if (__syncthreads_or(bad) && tid == 0) atomicOr(&rec[b].bad, 1);
     }
 }
@@ -218,9 +217,13 @@ cudaError_t launch_stream_step(adsc_ctx *c)
     const int nt = c->lay.ntiles;
     dim3 grid(nt, c->pb.B);
     Workspace &w = c->ws;
-    for (int s = 0; s < 4; ++s) {
-        double *const *in = (s == 0) ? w.U : (s == 2 ? w.Ub : w.Ua);
-        double *const *out = (s == 0 || s == 2) ? w.Ua : (s == 1 ? w.Ub : w.U);
+    double a_next[4], b_w[4];
+    rk_tableau(c->rk_order, c->pb.dt, a_next, b_w);
+    const int ns = c->rk_order, last = ns - 1;
+    for (int s = 0; s < ns; ++s) {
+        // stage states ping-pong between Ua and Ub; the first stage reads, the last one writes, the state U
+        double *const *in = (s == 0) ? w.U : ((s & 1) ? w.Ua : w.Ub);
+        double *const *out = (s == last) ? w.U : ((s & 1) ? w.Ub : w.Ua);
         if (!c->pb.fixed_bg) {
             k_stream_I<<<grid, GEN_THREADS, 0, c->stream>>>(c->pb, c->tb, in[0], in[1], w.dl, w.tot, w.rec, nt);
             k_stream_carry<<<c->pb.B, GEN_THREADS, 0, c->stream>>>(w.tot, w.carry, w.rec, nt);
@@ -228,7 +231,7 @@ cudaError_t launch_stream_step(adsc_ctx *c)
         }
         StageIO io;
         for (int v = 0; v < 3; ++v) { io.in[v] = in[v]; io.un[v] = w.U[v]; io.acc[v] = w.ACC[v]; io.out[v] = out[v]; }
-        k_stream_rhs<<<grid, GEN_THREADS, 0, c->stream>>>(c->pb, c->tb, io, w.dl, w.carry, w.rec, nt, s);
+        k_stream_rhs<<<grid, GEN_THREADS, 0, c->stream>>>(c->pb, c->tb, io, w.dl, w.carry, w.rec, nt, s, last, a_next[s], b_w[s]);
         c->launches += 1;
     }
     return cudaGetLastError();

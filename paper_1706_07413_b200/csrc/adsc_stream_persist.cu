@@ -94,6 +94,7 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
 
     const Problem &pb = prm.pb;
     const SPConsts &K = prm.k;
+    const int NS = K.ns, LS = K.ns - 1;      // Runge-Kutta stages (4; 3 or 2 for the rules of reading R25), last stage
     const int N = pb.N, G = prm.G, tid = threadIdx.x;
     const int gi = blockIdx.x / G, c = blockIdx.x - gi * G;
     if (gi >= prm.groups) return;
@@ -147,7 +148,7 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
         unsigned stage_ctr = 0;
 
         for (;;) {
-            for (int s = 0; s < 4; ++s, ++stage_ctr) {
+            for (int s = 0; s < NS; ++s, ++stage_ctr) {
                 const int par = (int)(stage_ctr & 1u);
                 double *mine = mb + ((size_t)par * G + c) * SP_MBOX;
                 // ---- publish: chunk total (+ top), collapse flag, state edges
@@ -351,7 +352,7 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                             const double2 *pa = reinterpret_cast<const double2 *>(prm.ACC[v] + row + i0);
 #pragma unroll
                             for (int q = 0; q < P; q += 2) { const double2 x = pa[q / 2]; acc[v][q] = x.x; acc[v][q + 1] = x.y; }
-                            if (s < 3) {
+                            if (s < LS) {
                                 const double2 *pu = reinterpret_cast<const double2 *>(prm.U[v] + row + i0);
 #pragma unroll
                                 for (int q = 0; q < P; q += 2) { const double2 y = pu[q / 2]; un[v][q] = y.x; un[v][q + 1] = y.y; }
@@ -410,7 +411,7 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                             const double u0 = ph[3 + q], u1 = pi[3 + q], u2 = a[q];
                             acc[0][q] = fma(b_w, kP, u0); acc[1][q] = fma(b_w, kQ, u1); acc[2][q] = fma(b_w, kAv, u2);
                             nP[q] = fma(a_next, kP, u0);  nQ[q] = fma(a_next, kQ, u1);  nA[q] = fma(a_next, kAv, u2);
-                        } else if (s < 3) {
+                        } else if (s < LS) {
                             acc[0][q] = fma(b_w, kP, acc[0][q]); acc[1][q] = fma(b_w, kQ, acc[1][q]); acc[2][q] = fma(b_w, kAv, acc[2][q]);
                             nP[q] = fma(a_next, kP, un[0][q]);   nQ[q] = fma(a_next, kQ, un[1][q]);   nA[q] = fma(a_next, kAv, un[2][q]);
                         } else {
@@ -431,7 +432,7 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                                 }
                             }
                         }
-                        if (s < 3) {
+                        if (s < LS) {
 #pragma unroll
                             for (int v = 0; v < 3; ++v) {
                                 double2 *pa = reinterpret_cast<double2 *>(prm.ACC[v] + row + i0);
@@ -520,8 +521,8 @@ cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
         k.kw[0] = -20.0 * koc; k.kw[1] = 15.0 * koc; k.kw[2] = -6.0 * koc; k.kw[3] = koc;
         k.hh = 0.5 * h; k.c25 = 25.0 * h / 48.0; k.c12 = 0.25 * h; k.c1 = h / 48.0;
         k.inv12h2 = 1.0 / (12.0 * h * h); k.c_org = 1.0 / (2.0 * h);
-        k.a_next[0] = 0.5 * dt; k.a_next[1] = 0.5 * dt; k.a_next[2] = dt; k.a_next[3] = 0.0;
-        k.b_w[0] = dt / 6.0; k.b_w[1] = dt / 3.0; k.b_w[2] = dt / 3.0; k.b_w[3] = dt / 6.0;
+        rk_tableau(c->rk_order, dt, k.a_next, k.b_w);
+        k.ns = c->rk_order;
         k.thr = c->pb.thr;
     }
     if (c->sp_ppt == 8) {

@@ -11,6 +11,7 @@ constexpr int SP_MBOX = 24;                        // doubles per chunk mailbox
 
 struct SPConsts {
     double d4c, kw[4], hh, c25, c12, c1, inv12h2, c_org, a_next[4], b_w[4], thr;
+    int ns;                          // Runge-Kutta stages: u_{s+1} = u^n + a_next[s] k_s, u^{n+1} = u^n + sum b_w[s] k_s
 };
 
 struct SPParams {

@@ -69,6 +69,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
 
     const Problem &pb = prm.pb;
     const SPConsts &K = prm.k;
+    const int NS = K.ns, LS = K.ns - 1;      // Runge-Kutta stages (4; 3 or 2 for the rules of reading R25), last stage
     const int N = pb.N, G = prm.G, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, col = tid + 1;
     const int gi = blockIdx.x / G, c = blockIdx.x - gi * G;
     if (gi >= prm.groups) return;
@@ -126,7 +127,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
         unsigned stage_ctr = 0;
 
         for (;;) {
-            for (int s = 0; s < 4; ++s, ++stage_ctr) {
+            for (int s = 0; s < NS; ++s, ++stage_ctr) {
                 const int par = (int)(stage_ctr & 1u);
                 double *mine = mb + ((size_t)par * G + c) * SP_MBOX;
                 // ---- publish: chunk total (+ top), collapse flag, state edges
@@ -382,7 +383,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                                 const double2 x = p0[p / 2], y = p1[p / 2];
                                 ac0[p] = x.x; ac0[p + 1] = x.y; ac1[p] = y.x; ac1[p + 1] = y.y;
                             }
-                            if (s < 3) {
+                            if (s < LS) {
                                 const double2 *q0 = reinterpret_cast<const double2 *>(prm.U[0] + row + i0);
                                 const double2 *q1 = reinterpret_cast<const double2 *>(prm.U[1] + row + i0);
 #pragma unroll
@@ -399,7 +400,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                             const double2 *pa = reinterpret_cast<const double2 *>(prm.ACC[2] + row + i0);
 #pragma unroll
                             for (int p = 0; p < P; p += 2) { if (i0 + p >= pb.NP) continue; const double2 x = pa[p / 2]; aa[p] = x.x; aa[p + 1] = x.y; }
-                            if (s < 3) {
+                            if (s < LS) {
                                 const double2 *pu = reinterpret_cast<const double2 *>(prm.U[2] + row + i0);
 #pragma unroll
                                 for (int p = 0; p < P; p += 2) { if (i0 + p >= pb.NP) continue; const double2 x = pu[p / 2]; ua[p] = x.x; ua[p + 1] = x.y; }
@@ -410,14 +411,14 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                             const int i = i0 + p;
                             const double kAv = (i == 0 || i >= N - 1) ? 0.0 : kA[p];        // eqs (8), (11)
                             if (s == 0) { aa[p] = fma(b_w, kAv, a[p]); nA[p] = fma(a_next, kAv, a[p]); }
-                            else if (s < 3) { aa[p] = fma(b_w, kAv, aa[p]); nA[p] = fma(a_next, kAv, ua[p]); }
+                            else if (s < LS) { aa[p] = fma(b_w, kAv, aa[p]); nA[p] = fma(a_next, kAv, ua[p]); }
                             else {
                                 nA[p] = fma(b_w, kAv, aa[p]);
                                 if (i <= N - 1 && l0 + p < cn && !(nA[p] >= K.thr)) bad = 1;   // a6
                             }
                             if (i > N - 1) { nA[p] = 0.0; aa[p] = 0.0; }
                         }
-                        if (s < 3) {
+                        if (s < LS) {
                             double2 *pa = reinterpret_cast<double2 *>(prm.ACC[2] + row + i0);
 #pragma unroll
                             for (int p = 0; p < P; p += 2) { if (i0 + p < pb.NP) pa[p / 2] = make_double2(aa[p], aa[p + 1]); }
@@ -471,7 +472,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                         if (s == 0) {
                             ac0[p] = fma(b_w, vP, uP[3 + p]); ac1[p] = fma(b_w, vQ, uQ[3 + p]);
                             nP[p] = fma(a_next, vP, uP[3 + p]); nQ[p] = fma(a_next, vQ, uQ[3 + p]);
-                        } else if (s < 3) {
+                        } else if (s < LS) {
                             ac0[p] = fma(b_w, vP, ac0[p]); ac1[p] = fma(b_w, vQ, ac1[p]);
                             nP[p] = fma(a_next, vP, un0[p]); nQ[p] = fma(a_next, vQ, un1[p]);
                         } else {
@@ -492,12 +493,12 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                                 }
                             }
                         }
-                        double2 *d0 = reinterpret_cast<double2 *>((s < 3 ? prm.ACC[0] : prm.U[0]) + row + i0);
-                        double2 *d1 = reinterpret_cast<double2 *>((s < 3 ? prm.ACC[1] : prm.U[1]) + row + i0);
+                        double2 *d0 = reinterpret_cast<double2 *>((s < LS ? prm.ACC[0] : prm.U[0]) + row + i0);
+                        double2 *d1 = reinterpret_cast<double2 *>((s < LS ? prm.ACC[1] : prm.U[1]) + row + i0);
 #pragma unroll
                         for (int p = 0; p < P; p += 2) {
                             if (i0 + p >= pb.NP) continue;
-                            if (s < 3) { d0[p / 2] = make_double2(ac0[p], ac0[p + 1]); d1[p / 2] = make_double2(ac1[p], ac1[p + 1]); }
+                            if (s < LS) { d0[p / 2] = make_double2(ac0[p], ac0[p + 1]); d1[p / 2] = make_double2(ac1[p], ac1[p + 1]); }
                             else { d0[p / 2] = make_double2(nP[p], nP[p + 1]); d1[p / 2] = make_double2(nQ[p], nQ[p + 1]); }
                         }
                     }

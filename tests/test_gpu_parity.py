@@ -395,3 +395,44 @@ def test_mode_energies_match_oracle(env, name, B, N, J, nsteps):
     lib = binding.load_library()
     assert lib.adsc_mode_energies(ens.h, 0, E.ctypes.data) == binding.ADSC_EINVAL
     assert lib.adsc_mode_energies(ens.h, 33, E.ctypes.data) == binding.ADSC_EINVAL
+
+
+# ------------------------------------------------- f2: second- and third-order Runge-Kutta (R25)
+
+@pytest.mark.parametrize("order,path,ppt,name,B,N,nsteps", [
+    (3, 1, 4, "cfg2", 3, 4097, 1000),      # the paper's production runs used RK3
+    (3, 1, 8, "cfg5", 3, 2049, 500),
+    (3, 3, None, "cfg5", 3, 2049, 500),
+    (2, 1, 4, "cfg5", 3, 2049, 500),
+    (2, 3, None, "cfg1", 1, 1025, 500),
+    (3, 1, 4, "cfg4", 1, 66699, 60),
+])
+def test_rk_orders_match_oracle(env, order, path, ppt, name, B, N, nsteps):
+    Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
+    ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=path, stream_ppt=ppt, rk_order=order)
+    assert ens.path[0] == path
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 8), rk_order=order).step(nsteps)
+    _compare(f, ev)
+    _bc_invariants(f)
+    assert (d["steps_done"] == nsteps).all() and (d["collapsed"] == 0).all()
+
+
+def test_rk3_auto_path_and_collapse(env):
+    """Order 3 on a member that would fit the resident kernel takes a streaming path; flags and collapse times
+    agree with the oracle's RK3 evolution."""
+    B, nsteps = 8, 3300
+    Phi, Pi, _ = env["inputs"].make("tcollapse", B=B)
+    ens, f, d = _gpu_run(env, Phi, Pi, nsteps, rk_order=3, a_resolve_period=0)
+    assert ens.path[0] in (1, 3)
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=8, rk_order=3).step(nsteps)
+    od = ev.diagnostics()
+    assert (d["collapsed"] == od["collapsed"]).all() and od["collapsed"].any()
+    for b in range(B):
+        if od["collapsed"][b]:
+            assert abs(d["t_collapse"][b] - od["t_collapse"][b]) <= ev.dt * (1 + 1e-12)
+    binding = env["binding"]
+    lib = binding.load_library()
+    h = lib.adsc_create(1025, 1, 0.25, 0.1)
+    assert lib.adsc_set_option(h, binding.ADSC_OPT_RK_ORDER, 5.0) == binding.ADSC_EINVAL
+    assert lib.adsc_set_option(h, binding.ADSC_OPT_RK_ORDER, 3.0) == 0 and lib.adsc_path(h, None) == 1
+    lib.adsc_destroy(h)
