@@ -84,8 +84,8 @@ extern "C" {
 #define ADSC_OPT_RK_ORDER            8  /* 4 (default): classical RK4; 3: Heun's third-order rule; 2:
                                           explicit midpoint ("second, third, and fourth order accurate
                                           Runge-Kutta"; tableaux are readings R12, R25).
-                                          Orders 2 and 3 run on the streaming paths (the resident
-                                          kernel is RK4 only).  Set it before adsc_bind.           */
+                                          All three step paths implement them (the fixed-background
+                                          build is RK4 only).  Set it before adsc_bind.            */
 
 typedef struct adsc_ctx *adsc_handle;
 

@@ -44,7 +44,7 @@ static void compute_layout(adsc_ctx *c)
 
 static void resolve_path(adsc_ctx *c)
 {
-    const bool can_res = (c->rk_order == 4) && resident_select(c);
+    const bool can_res = resident_select(c);
     if (c->path_opt == 1 || c->path_opt == 3) c->path = c->path_opt;
     else if (c->path_opt == 2) c->path = can_res ? 2 : 0;
     else c->path = can_res ? 2 : 1;
@@ -161,7 +161,7 @@ int adsc_set_option(adsc_handle h, int key, double value)
         if (!(value == 2.0 || value == 3.0 || value == 4.0)) return fail(h, ADSC_EINVAL, "Runge-Kutta order: 2, 3 or 4");
         if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_RK_ORDER before adsc_bind");
         h->rk_order = (int)value;
-        resolve_path(h);                 // the resident kernel is RK4 only: other orders take a streaming path
+        resolve_path(h);                 // (generation-1 and tuning configurations of the resident kernel are RK4 only)
         if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
         return ADSC_OK;
     case ADSC_OPT_STREAM_PPT:

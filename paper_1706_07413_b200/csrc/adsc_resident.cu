@@ -363,9 +363,10 @@ static const ResConfig &cfg_at(int k)
 {
     return k < n_cfgs3 ? g_cfgs3[k] : g_cfgs1[k - n_cfgs3];
 }
-static const void *fn_for(const ResConfig &g, int cl, int fixed_bg)
+static const void *fn_for(const ResConfig &g, int cl, int fixed_bg, int rk_order)
 {
-    const void *const *fn = fixed_bg ? g.fnf : g.fn;
+    if (fixed_bg && rk_order != 4) return nullptr;          // not compiled: takes a streaming path
+    const void *const *fn = fixed_bg ? g.fnf : (rk_order == 3 ? g.fn3 : rk_order == 2 ? g.fn2 : g.fn);
     if (cl == 1) return fn[0];
     if (g.any_cl) return fn[1];
     return cl == 2 ? fn[1] : cl == 4 ? fn[2] : cl == 8 ? fn[3] : nullptr;
@@ -384,7 +385,7 @@ bool resident_select(adsc_ctx *c)
         if (n_act % g.seg) continue;
         const int cl = n_act / g.seg;
         if (cl < 1 || cl > 8) continue;
-        if (!fn_for(g, cl, c->pb.fixed_bg)) continue;
+        if (!fn_for(g, cl, c->pb.fixed_bg, c->rk_order)) continue;
         if (c->dev_smem_optin > 0 && g.smem > (size_t)c->dev_smem_optin) continue;
         c->res_cfg = k; c->cluster = cl;
         return true;
@@ -395,7 +396,7 @@ bool resident_select(adsc_ctx *c)
 cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last)
 {
     const ResConfig &g = cfg_at(c->res_cfg);
-    const void *fn = fn_for(g, c->cluster, c->pb.fixed_bg);
+    const void *fn = fn_for(g, c->cluster, c->pb.fixed_bg, c->rk_order);
     if (!fn) return cudaErrorInvalidDeviceFunction;      // adsc_step checks this combination before launching
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem);
     if (e != cudaSuccess) return e;
@@ -410,8 +411,7 @@ cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last)
         k.kw[0] = -20.0 * koc; k.kw[1] = 15.0 * koc; k.kw[2] = -6.0 * koc; k.kw[3] = koc;
         k.hh = 0.5 * h; k.c25 = 25.0 * h / 48.0; k.c12 = 0.25 * h; k.c1 = h / 48.0;
         k.inv12h2 = 1.0 / (12.0 * h * h); k.c_org = 1.0 / (2.0 * h);
-        k.a_next[0] = 0.5 * dt; k.a_next[1] = 0.5 * dt; k.a_next[2] = dt; k.a_next[3] = 0.0;
-        k.b_w[0] = dt / 6.0; k.b_w[1] = dt / 3.0; k.b_w[2] = dt / 3.0; k.b_w[3] = dt / 6.0;
+        rk_tableau(c->rk_order, dt, k.a_next, k.b_w);
         k.thr = c->pb.thr;
     }
     cudaLaunchConfig_t cfg = {};

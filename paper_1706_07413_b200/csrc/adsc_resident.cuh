@@ -41,6 +41,8 @@ struct ResConfig {
     bool any_cl;
     const void *fn[4];
     const void *fnf[4];    // the same for the fixed background A = 1, delta = 0 (nullptr: not compiled)
+    const void *fn3[4];    // Runge-Kutta order 3 (Heun), dynamical metric
+    const void *fn2[4];    // Runge-Kutta order 2 (explicit midpoint), dynamical metric
 };
 
 // generation-3 table (adsc_resident3.cu); the generation-1 table is local to adsc_resident.cu

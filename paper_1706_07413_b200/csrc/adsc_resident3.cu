@@ -107,7 +107,9 @@ __device__ __forceinline__ void st_async_f64x2(uint32_t dst_cluster, double v0, 
 
 // FIXED: the paper's second workload (Table II), A = 1 and delta = 0 held fixed: no f', no scan,
 // no exponential, eq (4) not evolved, no collapse test -- the same stencils, exchanges and RK combine.
-template <int P, int THREADS, bool ACC_REG, int CL, bool FIXED>
+// NS: Runge-Kutta stages per step: 4 (classical RK4), 3 (Heun's third-order rule) or 2 (explicit midpoint): the
+// weights come in ResConsts (R12, R25); only the stage count and the barrier phase bookkeeping differ.
+template <int P, int THREADS, bool ACC_REG, int CL, bool FIXED, int NS>
 __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resident3(const __grid_constant__ ResParams prm)
 {
     using L = Res3Layout<P, THREADS, ACC_REG, CL>;
@@ -298,10 +300,13 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
 #pragma unroll 1
     for (long long n = 0; n < prm.nsteps; ++n) {
 #pragma unroll 1
-        for (int s = 0; s < 4; ++s) {
+        for (int s = 0; s < NS; ++s) {
+            // index of this stage's sync points since the kernel started; with four stages per step its low bits
+            // depend on s only
+            const unsigned j = (NS == 4) ? (unsigned)s : (unsigned)(n * NS + s);
             const double a_next = K.a_next[s], b_w = K.b_w[s];
             // sync S index j = 4n+s: buffer s&1; sync F index 4n+s: parity s&1
-            const double2 *wts = wt + (s & 1) * NG;
+            const double2 *wts = wt + (j & 1u) * NG;
 
             // ---------------------------------------------------------------- phase 1 (after sync S)
             double hlP[3], hrP[3], hlQ[3], hrQ[3];    // 3 halo points per side of the stage state
@@ -412,7 +417,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
             // a4/a5 for A (eq 4 needs no neighbour).  Invariant at the start of every step: acc == u^n == state.
             if constexpr (FIXED) {
                 // A is not evolved
-            } else if (s < 3) {
+            } else if (s < NS - 1) {
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
                     const int ui = (2 * P + p) * THREADS + tid;
@@ -448,7 +453,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                         kQ[0] = fma(8.0 * G1 - G2, K.c_org, qq);
                     }
                 }
-                if (s < 3) {
+                if (s < NS - 1) {
 #pragma unroll
                     for (int p = p0; p < p1; ++p) {
                         const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
@@ -474,7 +479,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
             // edge operands are taken before the interior state is overwritten (ph, pi are not flux inputs
             // any more at this point: H, F, G1, G2 hold everything phase 2 needs)
             if (EARLY) rhs_combine(2, P - 2);
-            mbar_wait<MULTI>(mbF, (uint32_t)(s & 1));                     // sync F: wait
+            mbar_wait<MULTI>(mbF, (uint32_t)(j & 1u));                    // sync F: wait
 
             // ---------------------------------------------------------------- phase 2
             {
@@ -493,9 +498,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
             }
             if (EARLY) { rhs_combine(0, 2); rhs_combine(P - 2, P); }
             else rhs_combine(0, P);
-            const int jb = (s + 1) & 1;                                   // buffer of the next sync S
-            publish_S(jb, s == 3);                                        // sync S: arrive
-            if (s < 3) {
+            const int jb = (int)((j + 1u) & 1u);                          // buffer of the next sync S
+            publish_S(jb, s == NS - 1);                                   // sync S: arrive
+            if (s < NS - 1) {
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
                     const int uP = (0 * P + p) * THREADS + tid, uQ = (1 * P + p) * THREADS + tid;
@@ -504,8 +509,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 }
             }
             ko_rest();                                                    // for the next stage
-            mbar_wait<MULTI>(jb ? mbS1 : mbS0, (uint32_t)(((s + 1) >> 1) & 1));   // sync S: wait
-            if (s == 3) {
+            mbar_wait<MULTI>(jb ? mbS1 : mbS0, (uint32_t)(((j + 1u) >> 1) & 1u));   // sync S: wait
+            if (s == NS - 1) {
                 // a6: collapse test of PAPER.md:85 on A^{n+1}: every warp of the member published its flag
                 int any = 0;
                 if constexpr (!FIXED) {
@@ -542,23 +547,33 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
 }
 
 // ------------------------------------------------------------------ configuration table
-#define ADSC_RES3_FN(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false>
-#define ADSC_RES3_FNF(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, true>
-// fn: dynamical A, delta; fnf: fixed background, nullptr where not compiled (tuning variants)
+#define ADSC_RES3_FN(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false, 4>
+#define ADSC_RES3_FNF(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, true, 4>
+#define ADSC_RES3_FN3(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false, 3>
+#define ADSC_RES3_FN2(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false, 2>
+// fn: dynamical A, delta, RK4; fnf: fixed background; fn3, fn2: Runge-Kutta orders 3 and 2 (R25);
+// nullptr where not compiled (tuning variants)
 #define ADSC_RES3_CFG_ALL(P_, T_, ACC_)                                                               \
     { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 8>::bytes, false,       \
       { ADSC_RES3_FN(P_, T_, ACC_, 1), ADSC_RES3_FN(P_, T_, ACC_, 2), ADSC_RES3_FN(P_, T_, ACC_, 4),    \
         ADSC_RES3_FN(P_, T_, ACC_, 8) },                                                              \
       { ADSC_RES3_FNF(P_, T_, ACC_, 1), ADSC_RES3_FNF(P_, T_, ACC_, 2), ADSC_RES3_FNF(P_, T_, ACC_, 4), \
-        ADSC_RES3_FNF(P_, T_, ACC_, 8) } }
+        ADSC_RES3_FNF(P_, T_, ACC_, 8) },                                                             \
+      { ADSC_RES3_FN3(P_, T_, ACC_, 1), ADSC_RES3_FN3(P_, T_, ACC_, 2), ADSC_RES3_FN3(P_, T_, ACC_, 4), \
+        ADSC_RES3_FN3(P_, T_, ACC_, 8) },                                                             \
+      { ADSC_RES3_FN2(P_, T_, ACC_, 1), ADSC_RES3_FN2(P_, T_, ACC_, 2), ADSC_RES3_FN2(P_, T_, ACC_, 4), \
+        ADSC_RES3_FN2(P_, T_, ACC_, 8) } }
 #define ADSC_RES3_CFG_ONE(P_, T_, ACC_)                                                               \
     { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 1>::bytes, false,       \
       { ADSC_RES3_FN(P_, T_, ACC_, 1), nullptr, nullptr, nullptr },                                   \
-      { ADSC_RES3_FNF(P_, T_, ACC_, 1), nullptr, nullptr, nullptr } }
+      { ADSC_RES3_FNF(P_, T_, ACC_, 1), nullptr, nullptr, nullptr },                                  \
+      { ADSC_RES3_FN3(P_, T_, ACC_, 1), nullptr, nullptr, nullptr },                                  \
+      { ADSC_RES3_FN2(P_, T_, ACC_, 1), nullptr, nullptr, nullptr } }
 #define ADSC_RES3_CFG_TUNE(P_, T_, ACC_)                                                              \
     { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 8>::bytes, false,       \
       { ADSC_RES3_FN(P_, T_, ACC_, 1), ADSC_RES3_FN(P_, T_, ACC_, 2), ADSC_RES3_FN(P_, T_, ACC_, 4),    \
         ADSC_RES3_FN(P_, T_, ACC_, 8) },                                                              \
+      { nullptr, nullptr, nullptr, nullptr }, { nullptr, nullptr, nullptr, nullptr },               \
       { nullptr, nullptr, nullptr, nullptr } }
 
 const ResConfig g_cfgs3[] = {

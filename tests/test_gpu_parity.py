@@ -406,6 +406,11 @@ def test_mode_energies_match_oracle(env, name, B, N, J, nsteps):
     (2, 1, 4, "cfg5", 3, 2049, 500),
     (2, 3, None, "cfg1", 1, 1025, 500),
     (3, 1, 4, "cfg4", 1, 66699, 60),
+    (3, 2, None, "cfg5", 6, 2049, 1000),   # resident kernel, stage count templated
+    (3, 2, None, "cfg2", 3, 4097, 1000),   # resident, cluster of 2
+    (3, 2, None, "cfg3", 2, 8193, 300),    # resident, cluster of 4
+    (2, 2, None, "cfg5", 3, 2049, 501),    # odd number of steps: barrier phases across steps
+    (2, 2, None, "cfg1", 1, 1025, 500),
 ])
 def test_rk_orders_match_oracle(env, order, path, ppt, name, B, N, nsteps):
     Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
@@ -418,12 +423,11 @@ def test_rk_orders_match_oracle(env, order, path, ppt, name, B, N, nsteps):
 
 
 def test_rk3_auto_path_and_collapse(env):
-    """Order 3 on a member that would fit the resident kernel takes a streaming path; flags and collapse times
-    agree with the oracle's RK3 evolution."""
+    """Order 3 on the resident kernel (auto path): flags and collapse times agree with the oracle's RK3 evolution."""
     B, nsteps = 8, 3300
     Phi, Pi, _ = env["inputs"].make("tcollapse", B=B)
     ens, f, d = _gpu_run(env, Phi, Pi, nsteps, rk_order=3, a_resolve_period=0)
-    assert ens.path[0] in (1, 3)
+    assert ens.path[0] == 2
     ev = env["oracle"].Evolution(Phi, Pi, nthreads=8, rk_order=3).step(nsteps)
     od = ev.diagnostics()
     assert (d["collapsed"] == od["collapsed"]).all() and od["collapsed"].any()
@@ -434,5 +438,5 @@ def test_rk3_auto_path_and_collapse(env):
     lib = binding.load_library()
     h = lib.adsc_create(1025, 1, 0.25, 0.1)
     assert lib.adsc_set_option(h, binding.ADSC_OPT_RK_ORDER, 5.0) == binding.ADSC_EINVAL
-    assert lib.adsc_set_option(h, binding.ADSC_OPT_RK_ORDER, 3.0) == 0 and lib.adsc_path(h, None) == 1
+    assert lib.adsc_set_option(h, binding.ADSC_OPT_RK_ORDER, 3.0) == 0 and lib.adsc_path(h, None) == 2
     lib.adsc_destroy(h)
