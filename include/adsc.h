@@ -158,6 +158,11 @@ int adsc_get_fields(adsc_handle h, double *d_Phi, double *d_Pi, double *d_A, dou
  * the getter, synchronises before returning. */
 int adsc_set_initial_host(adsc_handle h, const double *h_Phi, const double *h_Pi);
 int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta);
+/* The same without the final synchronisation: the copies are only ENQUEUED on the bound stream; the caller
+ * synchronises that stream (or calls adsc_diagnostics, which does) before reading the host buffers, which should
+ * be pinned for the copies to overlap other streams' work.  Lets sub-batches on different handles / streams
+ * pipeline their transfers against each other's kernels. */
+int adsc_get_fields_host_async(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta);
 
 /* Normal-mode spectrum of the current state ("the current numerical solution can be
  * decomposed into a spectrum of normal modes").  For the AdS4 modes e_j (R19),

@@ -62,6 +62,7 @@ _SIGS = {
     "adsc_set_initial_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_get_fields_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_mode_energies": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "adsc_get_fields_host_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_launch_count": (C.c_longlong, [C.c_void_p]),
     "adsc_path": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
     "adsc_last_error": (C.c_char_p, [C.c_void_p]),
@@ -151,6 +152,10 @@ def adsc_get_fields_host(h, h_Phi, h_Pi, h_A, h_delta):
 
 def adsc_mode_energies(h, J, host_out_ptr):
     _check(h, load_library().adsc_mode_energies(h, int(J), host_out_ptr))
+
+
+def adsc_get_fields_host_async(h, h_Phi, h_Pi, h_A, h_delta):
+    _check(h, load_library().adsc_get_fields_host_async(h, h_Phi, h_Pi, h_A, h_delta))
 
 
 def adsc_launch_count(h):
@@ -283,13 +288,15 @@ class Ensemble:
                             out["delta"].data_ptr() if delta else None)
         return out
 
-    def get_fields_host(self, delta=True, out=None):
+    def get_fields_host(self, delta=True, out=None, sync=True):
+        """sync=False only enqueues the copies (adsc_get_fields_host_async): synchronise the stream, or call
+        diagnostics(), before reading `out`."""
         keys = ("Phi", "Pi", "A", "delta") if delta else ("Phi", "Pi", "A")
         if out is None:
             out = {k: np.empty((self.batch, self.N)) for k in keys}
+        fn = adsc_get_fields_host if sync else adsc_get_fields_host_async
         with self.torch.cuda.device(self.device):
-            adsc_get_fields_host(self.h, *(self._host(out[k], k) if k in out else None
-                                           for k in ("Phi", "Pi", "A", "delta")))
+            fn(self.h, *(self._host(out[k], k) if k in out else None for k in ("Phi", "Pi", "A", "delta")))
         return out
 
     @property
@@ -299,3 +306,54 @@ class Ensemble:
     @property
     def path(self):
         return adsc_path(self.h)
+
+
+class PipelinedEnsemble:
+    """The same batch cut into `parts` contiguous sub-batches, each with its own handle, workspace and CUDA
+    stream, so that one sub-batch's host<->device transfers overlap another one's kernels (members are
+    independent: there is nothing to exchange).  Host-side interface only: set_initial / get_fields_host take HOST
+    arrays (pinned torch tensors overlap best) of shape [batch, N]; everything is enqueued asynchronously and
+    `synchronize()` / `diagnostics()` wait for it.  Argument marshalling only, like Ensemble."""
+
+    def __init__(self, N, batch, parts=2, device="cuda:0", **kw):
+        import torch
+        self.torch = torch
+        self.N, self.batch = int(N), int(batch)
+        parts = max(1, min(int(parts), self.batch))
+        edges = [self.batch * k // parts for k in range(parts + 1)]
+        self.ranges = [(edges[k], edges[k + 1]) for k in range(parts)]
+        self.device = torch.device(device)
+        self.streams = [torch.cuda.Stream(device=self.device) for _ in self.ranges]
+        self.parts = [Ensemble(N, hi - lo, device=device, stream=st, **kw)
+                      for (lo, hi), st in zip(self.ranges, self.streams)]
+        self.dt = self.parts[0].dt
+
+    def set_initial(self, Phi, Pi):
+        for e, (lo, hi) in zip(self.parts, self.ranges):
+            e.set_initial(Phi[lo:hi], Pi[lo:hi])
+        return self
+
+    def step(self, nsteps):
+        for e in self.parts:
+            e.step(nsteps)
+        return self
+
+    def get_fields_host(self, out, delta=False, sync=False):
+        for e, (lo, hi) in zip(self.parts, self.ranges):
+            e.get_fields_host(delta=delta, out={k: v[lo:hi] for k, v in out.items()}, sync=sync)
+        return out
+
+    def synchronize(self):
+        for st in self.streams:
+            st.synchronize()
+
+    def diagnostics(self):
+        return np.concatenate([e.diagnostics() for e in self.parts])
+
+    @property
+    def launch_count(self):
+        return sum(e.launch_count for e in self.parts)
+
+    def close(self):
+        for e in self.parts:
+            e.close()

@@ -339,7 +339,7 @@ int adsc_get_fields(adsc_handle h, double *d_Phi, double *d_Pi, double *d_A, dou
     return ADSC_OK;
 }
 
-int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta)
+static int get_fields_host_impl(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta, bool sync)
 {
     if (!h) return fail(nullptr, ADSC_EINVAL, "null handle");
     if (!h->bound || !h->have_state) return fail(h, ADSC_ESTATE, "adsc_bind and adsc_set_initial first");
@@ -356,8 +356,18 @@ int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A
         }
         ADSC_CUDA(cudaMemcpyAsync(dst[v], stage, n, cudaMemcpyDeviceToHost, h->stream), "D2H field");
     }
-    ADSC_CUDA(cudaStreamSynchronize(h->stream), "stream synchronize");
+    if (sync) ADSC_CUDA(cudaStreamSynchronize(h->stream), "stream synchronize");
     return ADSC_OK;
+}
+
+int adsc_get_fields_host(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta)
+{
+    return get_fields_host_impl(h, h_Phi, h_Pi, h_A, h_delta, true);
+}
+
+int adsc_get_fields_host_async(adsc_handle h, double *h_Phi, double *h_Pi, double *h_A, double *h_delta)
+{
+    return get_fields_host_impl(h, h_Phi, h_Pi, h_A, h_delta, false);
 }
 
 int adsc_mode_energies(adsc_handle h, int J, double *host_out)
