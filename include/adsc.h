@@ -105,6 +105,7 @@ typedef struct {
 
 /* Create a solver for `batch` members on N grid points.
  *   N        >= 9 and odd (Simpson needs N-1 even)
+ *   batch    1..65535 members (independent evolutions); N*batch <= 4e9
  *   courant  dt = courant*h, 0 < courant <= 1 (method-of-lines RK4)
  *   ko_eps   >= 0: Kreiss-Oliger coefficient of the 7-point dissipation added to the
  *            right-hand sides of Phi and Pi (BASELINE.json configs[0]; not in the paper)

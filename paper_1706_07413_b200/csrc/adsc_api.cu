@@ -74,7 +74,7 @@ extern "C" {
 adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
 {
     if (N < 9 || (N - 1) % 2 != 0) { g_create_error = "N must be >= 9 and odd"; return nullptr; }
-    if (batch < 1) { g_create_error = "batch must be >= 1"; return nullptr; }
+    if (batch < 1 || batch > 65535) { g_create_error = "batch must be in 1..65535 (grid.y of the pack/solve kernels)"; return nullptr; }
     if (!(courant > 0.0 && courant <= 1.0)) { g_create_error = "courant must be in (0,1]"; return nullptr; }
     if (!(ko_eps >= 0.0)) { g_create_error = "ko_eps must be >= 0"; return nullptr; }
     if ((double)N * (double)batch > 4.0e9) { g_create_error = "N*batch too large"; return nullptr; }

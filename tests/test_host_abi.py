@@ -58,7 +58,7 @@ def test_diag_struct_layout_matches_header(lib):
 
 def test_create_argument_checks_and_workspace_size(lib):
     for bad in ((8, 1, 0.25, 0.1), (10, 1, 0.25, 0.1), (1025, 0, 0.25, 0.1), (1025, 1, 0.0, 0.1),
-                (1025, 1, 1.5, 0.1), (1025, 1, 0.25, -1.0), (1025, 1, float("nan"), 0.1)):
+                (1025, 1, 1.5, 0.1), (1025, 1, 0.25, -1.0), (1025, 1, float("nan"), 0.1), (1025, 65536, 0.25, 0.1)):
         assert not lib.adsc_create(*bad), bad
         assert lib.adsc_last_error(None)
     h = lib.adsc_create(4097, 16, 0.25, 0.1)
