@@ -14,6 +14,8 @@
 //             E = e^{-delta}, fluxes G, H, F, D4 and Kreiss-Oliger stencils, RK combine, in-place
 //             write of the new stage state, running sum of the NEW state's f' for the next stage.
 // The discrete algorithm is DESIGN.md section 1; nothing here is shared with oracle/.
+#include <type_traits>
+
 #include "adsc_stream_persist.cuh"
 #include "adsc_exp.cuh"
 
@@ -211,13 +213,18 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                 double m2n[P + 2];                                            // -2 sc of my points in the coming tile
 #pragma unroll
                 for (int q = 0; q < P + 2; ++q) m2n[q] = -2.0 * tSC[min(ci0 + (ntile - 1) * SP_TILE + P * tid + q - 1, N - 1)];
-                for (int tt = ntile - 1; tt >= 0; --tt) {
+                // The tile body is compiled twice: EDGE = true is general (ragged tiles, the tiles at x = 0 and x = pi/2);
+                // EDGE = false is for full tiles at least 8 points away from both ends of the grid, where every mask
+                // and end-of-domain test below is a compile-time constant and disappears (2/3 of the instructions
+                // of the general body are such integer/predicate work).
+                auto tile_body = [&](auto edge_c, const int tt) {
+                    constexpr bool EDGE = decltype(edge_c)::value;
                     const int tl0 = tt * SP_TILE;
-                    const int tend = min(tl0 + SP_TILE, cn);
+                    const int tend = EDGE ? min(tl0 + SP_TILE, cn) : tl0 + SP_TILE;
                     const int l0 = tl0 + P * tid;
                     const int i0 = ci0 + l0;                              // global index of my first point
-                    const bool any = l0 < tend;
-                    const bool tile_hi_is_domain_end = (ci0 + tend == N); // the tile holds i = N-1
+                    const bool any = EDGE ? (l0 < tend) : true;
+                    const bool tile_hi_is_domain_end = EDGE && (ci0 + tend == N);   // the tile holds i = N-1
                     const bool last_thr = any && (l0 + P >= tend);   // owner of the tile's last point
 
                     // stage state: ph[r], pi[r] at l0 - 3 + r (r = 0..P+5), a at l0..l0+P-1
@@ -245,17 +252,20 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                     double m2sc[P], tT4[P], tC4[P];
                     const double m2m = m2n[0], m2p = m2n[P + 1];          // -2 sc at l0 - 1 and l0 + P
 #pragma unroll
-                    for (int q = 0; q < P; ++q) { m2sc[q] = m2n[1 + q]; tT4[q] = tT[min(i0 + q, N - 1)]; tC4[q] = tC[min(i0 + q, N - 1)]; }
+                    for (int q = 0; q < P; ++q) {
+                        const int it = EDGE ? min(i0 + q, N - 1) : i0 + q;
+                        m2sc[q] = m2n[1 + q]; tT4[q] = tT[it]; tC4[q] = tC[it];
+                    }
 
                     // a1: f' = -2 sc (Phi^2 + Pi^2) of my points (zero above i = N-2 and outside the chunk)
                     double fo[P], so[P];
 #pragma unroll
                     for (int q = 0; q < P; ++q) {
-                        const bool in = (l0 + q < cn) && (i0 + q <= N - 2);
+                        const bool in = !EDGE || ((l0 + q < cn) && (i0 + q <= N - 2));
                         fo[q] = (in && !FIXED) ? m2sc[q] * fma(ph[3 + q], ph[3 + q], pi[3 + q] * pi[3 + q]) : 0.0;
                     }
                     const double fm = m2m * fma(ph[2], ph[2], pi[2] * pi[2]);                             // f'_{l0-1}
-                    const double fp = (i0 + P <= N - 2) ? m2p * fma(ph[P + 3], ph[P + 3], pi[P + 3] * pi[P + 3]) : 0.0;   // f'_{l0+P}
+                    const double fp = (!EDGE || i0 + P <= N - 2) ? m2p * fma(ph[P + 3], ph[P + 3], pi[P + 3] * pi[P + 3]) : 0.0;   // f'_{l0+P}
                     so[P - 1] = fo[P - 1];
 #pragma unroll
                     for (int q = P - 2; q >= 0; --q) so[q] = so[q + 1] + fo[q];
@@ -292,14 +302,14 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                         kA[q] = FIXED ? 0.0 : (m2sc[q] * a[q]) * (Gv * pi[3 + q]);   // eq (4)
                         sH[sp_pad(2 + P * tid + q)] = Hx[2 + q];
                         sF[sp_pad(2 + P * tid + q)] = Fx[2 + q];
-                        if (i0 + q == 1) gE[0] = Gv;
-                        if (i0 + q == 2) gE[1] = Gv;
-                        if (i0 + q == N - 2) gE[2] = Gv;
-                        if (i0 + q == N - 3) gE[3] = Gv;
+                        if (EDGE && i0 + q == 1) gE[0] = Gv;
+                        if (EDGE && i0 + q == 2) gE[1] = Gv;
+                        if (EDGE && i0 + q == N - 2) gE[2] = Gv;
+                        if (EDGE && i0 + q == N - 3) gE[3] = Gv;
                     }
                     // fluxes at the two points below the tile (thread 0) ...
                     if (tid == 0) {
-                        if (i0 != 0) {                       // (at x = 0 the reader applies the parity rule)
+                        if (!EDGE || i0 != 0) {              // (at x = 0 the reader applies the parity rule)
                             const double f1 = fm;                                                             // f'_{l0-1}
                             const double f2 = eSC[6 * tt + 1] * fma(ph[1], ph[1], pi[1] * pi[1]);             // f'_{l0-2}
                             const double f3 = eSC[6 * tt] * fma(ph[0], ph[0], pi[0] * pi[0]);                 // f'_{l0-3}
@@ -311,9 +321,9 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                             const double g1 = ae1 * ph[2], g2 = ae2 * ph[1];
                             sH[sp_pad(1)] = ae1 * pi[2]; sH[sp_pad(0)] = ae2 * pi[1];
                             sF[sp_pad(1)] = eT[6 * tt + 2] * g1; sF[sp_pad(0)] = eT[6 * tt + 1] * g2;
-                            if (i0 - 1 == N - 2) gE[2] = g1;
-                            if (i0 - 1 == N - 3) gE[3] = g1;
-                            if (i0 - 2 == N - 3) gE[3] = g2;
+                            if (EDGE && i0 - 1 == N - 2) gE[2] = g1;
+                            if (EDGE && i0 - 1 == N - 3) gE[3] = g1;
+                            if (EDGE && i0 - 2 == N - 3) gE[3] = g2;
                         }
                     }
                     // ... and at the two points above it (owner of the tile's last point), unless the tile
@@ -321,12 +331,12 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                     if (last_thr && !tile_hi_is_domain_end) {
                         const int le = tend - tl0 + 2;                   // scratch slot of local index tend
                         const int ie = ci0 + tend;                       // its global index (<= N-1)
-                        if (ie == N - 1) {                   // H = 0 there; F by the limit of R5; then mirrored
+                        if (EDGE && ie == N - 1) {           // H = 0 there; F by the limit of R5; then mirrored
                             sH[sp_pad(le)] = 0.0;            sF[sp_pad(le)] = (16.0 * Gq[P - 1] - Gq[P - 2]) * K.inv12h2;
                             sH[sp_pad(le + 1)] = -Hx[P + 1]; sF[sp_pad(le + 1)] = Fx[P + 1];
                         } else {
-                            const double f1 = (ie + 1 <= N - 2) ? eSC[6 * (tt + 1) + 4] * fma(ph[P + 4], ph[P + 4], pi[P + 4] * pi[P + 4]) : 0.0;
-                            const double f2 = (ie + 2 <= N - 2) ? eSC[6 * (tt + 1) + 5] * fma(ph[P + 5], ph[P + 5], pi[P + 5] * pi[P + 5]) : 0.0;
+                            const double f1 = (!EDGE || ie + 1 <= N - 2) ? eSC[6 * (tt + 1) + 4] * fma(ph[P + 4], ph[P + 4], pi[P + 4] * pi[P + 4]) : 0.0;
+                            const double f2 = (!EDGE || ie + 2 <= N - 2) ? eSC[6 * (tt + 1) + 5] * fma(ph[P + 5], ph[P + 5], pi[P + 5] * pi[P + 5]) : 0.0;
                             double l0v = K.c25 * f1; l0v = fma(K.c12, fp, l0v); l0v = fma(-K.c1, fo[P - 1], l0v);
                             double l1v = K.c25 * f2; l1v = fma(K.c12, f1, l1v); l1v = fma(-K.c1, fp, l1v);
                             const double e0 = FIXED ? 1.0 : exp3_ref(fma(K.hh, B - fp - f1, l0v));
@@ -335,10 +345,10 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                             const double g0 = ae0 * ph[P + 3], g1 = ae1 * ph[P + 4];
                             sH[sp_pad(le)] = ae0 * pi[P + 3]; sH[sp_pad(le + 1)] = ae1 * pi[P + 4];
                             sF[sp_pad(le)] = eT[6 * (tt + 1) + 3] * g0; sF[sp_pad(le + 1)] = eT[6 * (tt + 1) + 4] * g1;
-                            if (ie == N - 3) gE[3] = g0;
-                            if (ie == N - 2) gE[2] = g0;
-                            if (ie + 1 == N - 3) gE[3] = g1;
-                            if (ie + 1 == N - 2) gE[2] = g1;
+                            if (EDGE && ie == N - 3) gE[3] = g0;
+                            if (EDGE && ie == N - 2) gE[2] = g0;
+                            if (EDGE && ie + 1 == N - 3) gE[3] = g1;
+                            if (EDGE && ie + 1 == N - 2) gE[2] = g1;
                         }
                     }
                     // global operands of the second half (cot^2/(12h), u^n, accumulator) and -2 sc of the next
@@ -368,10 +378,10 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                         Fx[0] = sF[sp_pad(sb)];             Fx[1] = sF[sp_pad(sb + 1)];
                         Hx[P + 2] = sH[sp_pad(sb + P + 2)]; Hx[P + 3] = sH[sp_pad(sb + P + 3)];
                         Fx[P + 2] = sF[sp_pad(sb + P + 2)]; Fx[P + 3] = sF[sp_pad(sb + P + 3)];
-                        if (i0 == 0) {                       // x = 0: H even, F odd (R2)
+                        if (EDGE && i0 == 0) {               // x = 0: H even, F odd (R2)
                             Hx[0] = Hx[4]; Hx[1] = Hx[3]; Fx[0] = -Fx[4]; Fx[1] = -Fx[3];
                         }
-                        if (any && i0 + P + 1 >= N - 1) {    // my window l0-2 .. l0+P+1 reaches i = N-1
+                        if (EDGE && any && i0 + P + 1 >= N - 1) {    // my window l0-2 .. l0+P+1 reaches i = N-1
                             const double lim = (16.0 * gE[2] - gE[3]) * K.inv12h2;   // F_{N-1} (R5)
 #pragma unroll
                             for (int k = 2; k < P + 4; ++k) {
@@ -401,11 +411,11 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                         double kP = fma(K.d4c, dH, qP);
                         double kQ = fma(tC4[q] * K.d4c, dF, qQ);
                         double kAv = kA[q];
-                        if (i == 0) {                        // eqs (7), (8); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
+                        if (EDGE && i == 0) {                // eqs (7), (8); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
                             kP = 0.0; kAv = 0.0;
                             kQ = fma(8.0 * gE[0] - gE[1], K.c_org, qQ);
                         }
-                        if (i >= N - 1) { kP = 0.0; kQ = 0.0; kAv = 0.0; }        // eqs (9)-(11)
+                        if (EDGE && i >= N - 1) { kP = 0.0; kQ = 0.0; kAv = 0.0; }   // eqs (9)-(11)
                         // a5: RK combine
                         if (s == 0) {
                             const double u0 = ph[3 + q], u1 = pi[3 + q], u2 = a[q];
@@ -416,19 +426,19 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                             nP[q] = fma(a_next, kP, un[0][q]);   nQ[q] = fma(a_next, kQ, un[1][q]);   nA[q] = fma(a_next, kAv, un[2][q]);
                         } else {
                             nP[q] = fma(b_w, kP, acc[0][q]); nQ[q] = fma(b_w, kQ, acc[1][q]); nA[q] = fma(b_w, kAv, acc[2][q]);
-                            if (!FIXED && i <= N - 1 && l0 + q < cn && !(nA[q] >= K.thr)) bad = 1;   // a6
+                            if (!FIXED && (!EDGE || (i <= N - 1 && l0 + q < cn)) && !(nA[q] >= K.thr)) bad = 1;   // a6
                         }
-                        if (i > N - 1) { nP[q] = 0.0; nQ[q] = 0.0; nA[q] = 0.0; acc[0][q] = 0.0; acc[1][q] = 0.0; acc[2][q] = 0.0; }
+                        if (EDGE && i > N - 1) { nP[q] = 0.0; nQ[q] = 0.0; nA[q] = 0.0; acc[0][q] = 0.0; acc[1][q] = 0.0; acc[2][q] = 0.0; }
                     }
                     if (any) {
 #pragma unroll
                         for (int q = 0; q < P; ++q) {
-                            if (l0 + q < cn) {
+                            if (!EDGE || l0 + q < cn) {
                                 Sv(0, l0 + q) = nP[q]; Sv(1, l0 + q) = nQ[q]; Sv(2, l0 + q) = nA[q];
-                                if (!FIXED && i0 + q <= N - 2) {   // f' of the new stage state, for the next publish
+                                if (!FIXED && (!EDGE || i0 + q <= N - 2)) {   // f' of the new stage state, for the next publish
                                     const double f = m2sc[q] * fma(nP[q], nP[q], nQ[q] * nQ[q]);
                                     facc += f;
-                                    if (i0 + q == N - 2) misc[1] = f * (1.0 / 12.0);
+                                    if (EDGE && i0 + q == N - 2) misc[1] = f * (1.0 / 12.0);
                                 }
                             }
                         }
@@ -452,6 +462,13 @@ __global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__
                         }
                     }
                     carry += ttot;
+                };   // tile_body
+                for (int tt = ntile - 1; tt >= 0; --tt) {
+                    // full tile, 8 points clear of x = 0 and of x = pi/2 (uniform over the CTA)
+                    const bool interior = (tt + 1) * SP_TILE <= cn && ci0 + tt * SP_TILE >= 8
+                                          && ci0 + (tt + 1) * SP_TILE + 8 <= N - 1;
+                    if (interior) tile_body(std::false_type{}, tt);
+                    else tile_body(std::true_type{}, tt);
                 }   // tiles
                 bad = __syncthreads_or(bad);
             }   // stages
