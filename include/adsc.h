@@ -67,8 +67,9 @@ extern "C" {
 #define ADSC_OPT_STREAM_PPT          6  /* tuning: contiguous points per thread of the persistent
                                           streaming kernel: 4 (256 threads per CTA, 1024-point
                                           tiles; default), 2 (512 threads) or 8 (224 threads,
-                                          1792-point tiles, register-blocked tile body; no
-                                          fixed-background build, 4 is used instead).  Results do
+                                          1792-point tiles, register-blocked tile body) or 84 (that
+                                          tile body with 4 points x 256 threads); 8 and 84 have no
+                                          fixed-background build (4 is used instead).  Results do
                                           not depend on it beyond rounding order.               */
 
 #define ADSC_OPT_FIXED_BACKGROUND    7  /* 1: evolve on the fixed background A = 1, delta = 0 (the

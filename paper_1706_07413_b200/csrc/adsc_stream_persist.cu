@@ -503,7 +503,8 @@ bool stream_persist_select(adsc_ctx *c)
     if (G > gmax) G = gmax;
     if (G < gmin) G = gmin;
     if (c->pb.fixed_bg && c->sp_ppt == 8) c->sp_ppt = 4;     // the 8-point kernel has no fixed-background build
-    if (c->sp_ppt != 2 && c->sp_ppt != 4 && c->sp_ppt != 8) c->sp_ppt = 8;
+    if ((c->pb.fixed_bg) && c->sp_ppt == 84) c->sp_ppt = 4;
+    if (c->sp_ppt != 2 && c->sp_ppt != 4 && c->sp_ppt != 8 && c->sp_ppt != 84) c->sp_ppt = 4;
     const int al = (c->sp_ppt == 8) ? 8 : 4;                 // chunks start on a thread boundary
     int Lc = ((N + G - 1) / G + al - 1) / al * al;
     G = (N + Lc - 1) / Lc;
@@ -542,7 +543,7 @@ cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
         k.ns = c->rk_order;
         k.thr = c->pb.thr;
     }
-    if (c->sp_ppt == 8) {
+    if (c->sp_ppt == 8 || c->sp_ppt == 84) {
         e = launch_stream_persist8(c, prm);
         c->launches++;
         return e;

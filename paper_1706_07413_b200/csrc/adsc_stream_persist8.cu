@@ -6,24 +6,22 @@
 // fluxes kept in registers and only two flux values per thread edge exchanged through shared memory, TWO
 // CTA barriers per tile (scan totals; flux edges) instead of three per 1024 points.
 // Equations: eqs (2)-(6); boundary conditions PAPER.md:59-75; algorithm DESIGN.md 1 and 6.
+#include <type_traits>
+
 #include "adsc_stream_persist.cuh"
 #include "adsc_exp.cuh"
 
 namespace adsc {
 
-constexpr int S8_P = 8;
-constexpr int S8_T = 224;                          // threads per CTA (7 warps)
-constexpr int S8_NW = S8_T / 32;
-constexpr int S8_TILE = S8_P * S8_T;               // 1792
-constexpr int S8_TILES = SP_CAP / S8_TILE;         // 4
-constexpr int S8_LD = S8_T + 2;                    // flux edge rows: one halo column per side
-static_assert(S8_TILE * S8_TILES == SP_CAP, "four tiles of 1792 points per chunk");
-
-struct S8Layout {
+// One compiled shape: P contiguous points per thread, T threads, tiles of P*T points, SP_CAP/(P*T) tiles per chunk.
+template <int P_, int T_>
+struct S8Cfg {
+    static constexpr int P = P_, T = T_, NW = T_ / 32, TILE = P_ * T_, TILES = SP_CAP / (P_ * T_), LD = T_ + 2;
+    static_assert(TILE * TILES == SP_CAP && T_ % 32 == 0 && P_ >= 4 && P_ % 2 == 0, "tiles must fill the 7168-point chunk");
     static constexpr int o_S = 0;                              // [3][SP_CAP], tile-wise [p][thread]
     static constexpr int o_xH = o_S + 3 * SP_CAP;              // [4][LD]: H at the first two / last two points of each thread
-    static constexpr int o_xF = o_xH + 4 * S8_LD;
-    static constexpr int o_lo = o_xF + 4 * S8_LD;              // chunk's lower halo: Phi[3], Pi[3], A[2] at l = -3..-1 / -2..-1
+    static constexpr int o_xF = o_xH + 4 * LD;
+    static constexpr int o_lo = o_xF + 4 * LD;                 // chunk's lower halo: Phi[3], Pi[3], A[2] at l = -3..-1 / -2..-1
     static constexpr int o_up = o_lo + 8;                      // [2]{Phi[3], Pi[3], A[2]} above the tile (ping-pong by tile)
     static constexpr int o_upf = o_up + 16;                    // [2]{H, H, F, F} at the two points above the tile (ping-pong)
     static constexpr int o_wt = o_upf + 8;                     // [2][8] warp totals (ping-pong by tile)
@@ -31,18 +29,18 @@ struct S8Layout {
     static constexpr int o_gE = o_sw + 8;                      // G_1, G_2, G_{N-2}, G_{N-3}
     static constexpr int o_misc = o_gE + 4;                    // carry, top, flags
     static constexpr int o_eSC = o_misc + 8;                   // -2 sc at every tile boundary -3..+2
-    static constexpr int o_eT = o_eSC + 6 * (S8_TILES + 1);    // tan^2 x likewise
-    static constexpr int n_doubles = o_eT + 6 * (S8_TILES + 1);
+    static constexpr int o_eT = o_eSC + 6 * (TILES + 1);       // tan^2 x likewise
+    static constexpr int n_doubles = o_eT + 6 * (TILES + 1);
     static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
+    // position of chunk-local index l (0 <= l < SP_CAP) inside a state array
+    __device__ static __forceinline__ int pos(int l)
+    {
+        const int tile = l / TILE, r = l - tile * TILE;
+        return tile * TILE + (r % P) * T + (r / P);
+    }
 };
 
-// position of chunk-local index l (0 <= l < SP_CAP) inside a state array
-__device__ __forceinline__ int s8_pos(int l)
-{
-    const int tile = l / S8_TILE, r = l - tile * S8_TILE;
-    return tile * S8_TILE + (r & 7) * S8_T + (r >> 3);
-}
-
+template <int NW>
 __device__ __forceinline__ double s8_block_sum(double v, double *sw)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -53,14 +51,15 @@ __device__ __forceinline__ double s8_block_sum(double v, double *sw)
     __syncthreads();
     double t = 0.0;
 #pragma unroll
-    for (int w = 0; w < S8_NW; ++w) t += sw[w];
+    for (int w = 0; w < NW; ++w) t += sw[w];
     return t;
 }
 
-__global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_constant__ SPParams prm)
+template <int P_, int T_>
+__global__ void __launch_bounds__(T_, 1) k_stream_persist8(const __grid_constant__ SPParams prm)
 {
-    using L = S8Layout;
-    constexpr int P = S8_P, T = S8_T, NW = S8_NW, LD = S8_LD;
+    using L = S8Cfg<P_, T_>;
+    constexpr int P = L::P, T = L::T, NW = L::NW, LD = L::LD, S8_TILE = L::TILE;
     constexpr unsigned FULL = 0xffffffffu;
     extern __shared__ __align__(16) double smem[];
     double *S = smem + L::o_S, *xH = smem + L::o_xH, *xF = smem + L::o_xF, *lo = smem + L::o_lo;
@@ -83,7 +82,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
     const double *__restrict__ tSC = prm.tb.sc;
     const double *__restrict__ tT = prm.tb.T;
     const double *__restrict__ tC = prm.tb.C;
-    auto Sg = [&](int v, int l) -> double & { return S[v * SP_CAP + s8_pos(l)]; };     // 0 <= l < cn
+    auto Sg = [&](int v, int l) -> double & { return S[v * SP_CAP + L::pos(l)]; };     // 0 <= l < cn
 
     // value of field v at chunk-local index l for the edge threads of a tile: below the chunk from `lo`, at and
     // above the tile end from `upb` (the tile above already holds the new stage state), else from the state array
@@ -131,7 +130,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                 const int par = (int)(stage_ctr & 1u);
                 double *mine = mb + ((size_t)par * G + c) * SP_MBOX;
                 // ---- publish: chunk total (+ top), collapse flag, state edges
-                double tot = s8_block_sum(facc, sw);
+                double tot = s8_block_sum<NW>(facc, sw);
                 if (owns_top) tot += misc[1];
                 if (tid == 0) { mine[0] = tot; mine[1] = bad ? 1.0 : 0.0; }
                 if (tid < 3) {
@@ -193,15 +192,19 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
 #pragma unroll
                 for (int q = 0; q < P + 2; ++q)
                     m2n[q] = -2.0 * tSC[min(ci0 + (ntile - 1) * S8_TILE + P * tid + q - 1, N - 1)];
-                for (int tt = ntile - 1; tt >= 0; --tt) {
+                // The tile body is compiled twice: EDGE = true is general (ragged tiles, the tiles at x = 0 and x = pi/2);
+                // EDGE = false is for full tiles at least 8 points away from both ends of the grid, where every mask
+                // and end-of-domain test below is a compile-time constant and disappears.
+                auto tile_body = [&](auto edge_c, const int tt) {
+                    constexpr bool EDGE = decltype(edge_c)::value;
                     const int tl0 = tt * S8_TILE;
-                    const int tend = min(tl0 + S8_TILE, cn);
+                    const int tend = EDGE ? min(tl0 + S8_TILE, cn) : tl0 + S8_TILE;
                     const int l0 = tl0 + P * tid;
                     const int i0 = ci0 + l0;                              // global index of my first point
-                    const bool any = l0 < tend;
+                    const bool any = EDGE ? (l0 < tend) : true;
                     const int nact = (tend - tl0 + P - 1) / P;            // threads that own a point of this tile
                     const bool last_thr = (tid == nact - 1);
-                    const bool tile_hi_is_domain_end = (ci0 + tend == N); // the tile holds i = N-1
+                    const bool tile_hi_is_domain_end = EDGE && (ci0 + tend == N);   // the tile holds i = N-1
                     const double *upb = up + 8 * (tt & 1);                // old values above this tile
                     const double *Sb = S + tl0 + tid;                     // (p = 0, my column) of this tile
 
@@ -228,21 +231,33 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                         upn[3] = uQ[3]; upn[4] = uQ[4]; upn[5] = uQ[5];
                         upn[6] = a[0];  upn[7] = a[1];
                     }
+                    // u^n and accumulator of A: issued now, used after the fluxes (eq (4) is combined before barrier F)
+                    double ua[P], aa[P];
+                    if (any && s > 0) {
+                        const double2 *pa = reinterpret_cast<const double2 *>(prm.ACC[2] + row + i0);
+#pragma unroll
+                        for (int p = 0; p < P; p += 2) { if (EDGE && i0 + p >= pb.NP) continue; const double2 x = pa[p / 2]; aa[p] = x.x; aa[p + 1] = x.y; }
+                        if (s < LS) {
+                            const double2 *pu = reinterpret_cast<const double2 *>(prm.U[2] + row + i0);
+#pragma unroll
+                            for (int p = 0; p < P; p += 2) { if (EDGE && i0 + p >= pb.NP) continue; const double2 x = pu[p / 2]; ua[p] = x.x; ua[p + 1] = x.y; }
+                        }
+                    }
                     // coefficient tables of my points: -2 sc was fetched during the previous tile
                     double m2sc[P], tT8[P];
                     const double m2m = m2n[0], m2p = m2n[P + 1];
 #pragma unroll
-                    for (int p = 0; p < P; ++p) { m2sc[p] = m2n[1 + p]; tT8[p] = tT[min(i0 + p, N - 1)]; }
+                    for (int p = 0; p < P; ++p) { m2sc[p] = m2n[1 + p]; tT8[p] = tT[EDGE ? min(i0 + p, N - 1) : i0 + p]; }
 
                     // a1: f' = -2 sc (Phi^2 + Pi^2) of my points (zero above i = N-2 and outside the chunk)
                     double fo[P], so[P];
 #pragma unroll
                     for (int p = 0; p < P; ++p) {
-                        const bool in = (l0 + p < cn) && (i0 + p <= N - 2);
+                        const bool in = !EDGE || ((l0 + p < cn) && (i0 + p <= N - 2));
                         fo[p] = in ? m2sc[p] * fma(uP[3 + p], uP[3 + p], uQ[3 + p] * uQ[3 + p]) : 0.0;
                     }
                     const double fm = m2m * fma(uP[2], uP[2], uQ[2] * uQ[2]);                                  // f'_{l0-1}
-                    const double fp = (i0 + P <= N - 2) ? m2p * fma(uP[P + 3], uP[P + 3], uQ[P + 3] * uQ[P + 3]) : 0.0;
+                    const double fp = (!EDGE || i0 + P <= N - 2) ? m2p * fma(uP[P + 3], uP[P + 3], uQ[P + 3] * uQ[P + 3]) : 0.0;
                     so[P - 1] = fo[P - 1];
 #pragma unroll
                     for (int p = P - 2; p >= 0; --p) so[p] = so[p + 1] + fo[p];
@@ -305,8 +320,8 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                         if (p == 2) G2 = Gv;
                         if (p == P - 1) Gl1 = Gv;
                         if (p == P - 2) Gl2 = Gv;
-                        if (i0 + p == N - 2) gE[2] = Gv;
-                        if (i0 + p == N - 3) gE[3] = Gv;
+                        if (EDGE && i0 + p == N - 2) gE[2] = Gv;
+                        if (EDGE && i0 + p == N - 3) gE[3] = Gv;
                     }
                     // flux edges of every thread: rows 0, 1 = first two points, rows 2, 3 = last two
                     xH[0 * LD + col] = H[0]; xH[1 * LD + col] = H[1]; xH[2 * LD + col] = H[P - 2]; xH[3 * LD + col] = H[P - 1];
@@ -314,7 +329,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                     if (tid == 0) {
                         // fluxes at the two points below the tile (column 0, rows 2, 3); at x = 0 the reader mirrors
                         double h1 = 0.0, h2 = 0.0, f1v = 0.0, f2v = 0.0, g1 = 0.0, g2 = 0.0;
-                        if (i0 != 0) {
+                        if (!EDGE || i0 != 0) {
                             const double f1 = fm;                                                          // f'_{l0-1}
                             const double f2 = eSC[6 * tt + 1] * fma(uP[1], uP[1], uQ[1] * uQ[1]);          // f'_{l0-2}
                             const double f3 = eSC[6 * tt] * fma(uP[0], uP[0], uQ[0] * uQ[0]);              // f'_{l0-3}
@@ -327,13 +342,13 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                             h1 = ae1 * uQ[2]; h2 = ae2 * uQ[1];
                             f1v = eT[6 * tt + 2] * g1; f2v = eT[6 * tt + 1] * g2;
                             xH[3 * LD] = h1; xH[2 * LD] = h2; xF[3 * LD] = f1v; xF[2 * LD] = f2v;
-                            if (i0 - 1 == N - 2) gE[2] = g1;
-                            if (i0 - 1 == N - 3) gE[3] = g1;
-                            if (i0 - 2 == N - 3) gE[3] = g2;
+                            if (EDGE && i0 - 1 == N - 2) gE[2] = g1;
+                            if (EDGE && i0 - 1 == N - 3) gE[3] = g1;
+                            if (EDGE && i0 - 2 == N - 3) gE[3] = g2;
                         }
                         // my first two fluxes are the upper halo of the next (lower) tile
                         double *ufn = upf + 4 * ((tt & 1) ^ 1);
-                        if (i0 == N - 1) {           // H = 0 at x = pi/2, F by the limit of R5, then mirrored (R3)
+                        if (EDGE && i0 == N - 1) {   // H = 0 at x = pi/2, F by the limit of R5, then mirrored (R3)
                             ufn[0] = 0.0; ufn[1] = -h1; ufn[2] = (16.0 * g1 - g2) * K.inv12h2; ufn[3] = f1v;
                         } else { ufn[0] = H[0]; ufn[1] = H[1]; ufn[2] = F[0]; ufn[3] = F[1]; }
                     }
@@ -347,8 +362,8 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                             hh0 = uf[0]; hh1 = uf[1]; ff0 = uf[2]; ff1 = uf[3];
                         } else {
                             const int ie = ci0 + tend;                   // < N-1 here (the top chunk never takes this path)
-                            const double f1 = (ie + 1 <= N - 2) ? eSC[6 * (tt + 1) + 4] * fma(uP[P + 4], uP[P + 4], uQ[P + 4] * uQ[P + 4]) : 0.0;
-                            const double f2 = (ie + 2 <= N - 2) ? eSC[6 * (tt + 1) + 5] * fma(uP[P + 5], uP[P + 5], uQ[P + 5] * uQ[P + 5]) : 0.0;
+                            const double f1 = (!EDGE || ie + 1 <= N - 2) ? eSC[6 * (tt + 1) + 4] * fma(uP[P + 4], uP[P + 4], uQ[P + 4] * uQ[P + 4]) : 0.0;
+                            const double f2 = (!EDGE || ie + 2 <= N - 2) ? eSC[6 * (tt + 1) + 5] * fma(uP[P + 5], uP[P + 5], uQ[P + 5] * uQ[P + 5]) : 0.0;
                             double l0v = K.c25 * f1; l0v = fma(K.c12, fp, l0v); l0v = fma(-K.c1, fo[P - 1], l0v);
                             double l1v = K.c25 * f2; l1v = fma(K.c12, f1, l1v); l1v = fma(-K.c1, fp, l1v);
                             const double e0 = exp3_ref(fma(K.hh, B - fp - f1, l0v));
@@ -357,10 +372,10 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                             const double g0 = ae0 * uP[P + 3], g1 = ae1 * uP[P + 4];
                             hh0 = ae0 * uQ[P + 3]; hh1 = ae1 * uQ[P + 4];
                             ff0 = eT[6 * (tt + 1) + 3] * g0; ff1 = eT[6 * (tt + 1) + 4] * g1;
-                            if (ie == N - 3) gE[3] = g0;
-                            if (ie == N - 2) gE[2] = g0;
-                            if (ie + 1 == N - 3) gE[3] = g1;
-                            if (ie + 1 == N - 2) gE[2] = g1;
+                            if (EDGE && ie == N - 3) gE[3] = g0;
+                            if (EDGE && ie == N - 2) gE[2] = g0;
+                            if (EDGE && ie + 1 == N - 3) gE[3] = g1;
+                            if (EDGE && ie + 1 == N - 2) gE[2] = g1;
                         }
                         xH[0 * LD + col + 1] = hh0; xH[1 * LD + col + 1] = hh1;
                         xF[0 * LD + col + 1] = ff0; xF[1 * LD + col + 1] = ff1;
@@ -370,7 +385,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                     // -2 sc of the next tile
                     double tC8[P], un0[P], un1[P], ac0[P], ac1[P], nA[P];
 #pragma unroll
-                    for (int p = 0; p < P; ++p) tC8[p] = tC[min(i0 + p, N - 1)];
+                    for (int p = 0; p < P; ++p) tC8[p] = tC[EDGE ? min(i0 + p, N - 1) : i0 + p];
 #pragma unroll
                     for (int q = 0; q < P + 2; ++q) m2n[q] = -2.0 * tSC[max(i0 + q - 1 - S8_TILE, -1)];
                     if (any) {
@@ -379,7 +394,7 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                             const double2 *p1 = reinterpret_cast<const double2 *>(prm.ACC[1] + row + i0);
 #pragma unroll
                             for (int p = 0; p < P; p += 2) {
-                                if (i0 + p >= pb.NP) continue;           // (rows are padded to a multiple of 4 only)
+                                if (EDGE && i0 + p >= pb.NP) continue;           // (rows are padded to a multiple of 4 only)
                                 const double2 x = p0[p / 2], y = p1[p / 2];
                                 ac0[p] = x.x; ac0[p + 1] = x.y; ac1[p] = y.x; ac1[p + 1] = y.y;
                             }
@@ -388,44 +403,33 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                                 const double2 *q1 = reinterpret_cast<const double2 *>(prm.U[1] + row + i0);
 #pragma unroll
                                 for (int p = 0; p < P; p += 2) {
-                                    if (i0 + p >= pb.NP) continue;
+                                    if (EDGE && i0 + p >= pb.NP) continue;
                                     const double2 x = q0[p / 2], y = q1[p / 2];
                                     un0[p] = x.x; un0[p + 1] = x.y; un1[p] = y.x; un1[p + 1] = y.y;
                                 }
                             }
                         }
                         // a4/a5 for A
-                        double ua[P], aa[P];
-                        if (s > 0) {
-                            const double2 *pa = reinterpret_cast<const double2 *>(prm.ACC[2] + row + i0);
-#pragma unroll
-                            for (int p = 0; p < P; p += 2) { if (i0 + p >= pb.NP) continue; const double2 x = pa[p / 2]; aa[p] = x.x; aa[p + 1] = x.y; }
-                            if (s < LS) {
-                                const double2 *pu = reinterpret_cast<const double2 *>(prm.U[2] + row + i0);
-#pragma unroll
-                                for (int p = 0; p < P; p += 2) { if (i0 + p >= pb.NP) continue; const double2 x = pu[p / 2]; ua[p] = x.x; ua[p + 1] = x.y; }
-                            }
-                        }
 #pragma unroll
                         for (int p = 0; p < P; ++p) {
                             const int i = i0 + p;
-                            const double kAv = (i == 0 || i >= N - 1) ? 0.0 : kA[p];        // eqs (8), (11)
+                            const double kAv = (EDGE && (i == 0 || i >= N - 1)) ? 0.0 : kA[p];   // eqs (8), (11)
                             if (s == 0) { aa[p] = fma(b_w, kAv, a[p]); nA[p] = fma(a_next, kAv, a[p]); }
                             else if (s < LS) { aa[p] = fma(b_w, kAv, aa[p]); nA[p] = fma(a_next, kAv, ua[p]); }
                             else {
                                 nA[p] = fma(b_w, kAv, aa[p]);
-                                if (i <= N - 1 && l0 + p < cn && !(nA[p] >= K.thr)) bad = 1;   // a6
+                                if ((!EDGE || (i <= N - 1 && l0 + p < cn)) && !(nA[p] >= K.thr)) bad = 1;   // a6
                             }
-                            if (i > N - 1) { nA[p] = 0.0; aa[p] = 0.0; }
+                            if (EDGE && i > N - 1) { nA[p] = 0.0; aa[p] = 0.0; }
                         }
                         if (s < LS) {
                             double2 *pa = reinterpret_cast<double2 *>(prm.ACC[2] + row + i0);
 #pragma unroll
-                            for (int p = 0; p < P; p += 2) { if (i0 + p < pb.NP) pa[p / 2] = make_double2(aa[p], aa[p + 1]); }
+                            for (int p = 0; p < P; p += 2) { if (!EDGE || i0 + p < pb.NP) pa[p / 2] = make_double2(aa[p], aa[p + 1]); }
                         } else {
                             double2 *pu = reinterpret_cast<double2 *>(prm.U[2] + row + i0);
 #pragma unroll
-                            for (int p = 0; p < P; p += 2) { if (i0 + p < pb.NP) pu[p / 2] = make_double2(nA[p], nA[p + 1]); }
+                            for (int p = 0; p < P; p += 2) { if (!EDGE || i0 + p < pb.NP) pu[p / 2] = make_double2(nA[p], nA[p + 1]); }
                         }
                     }
                     __syncthreads();                                      // barrier F: flux edges visible
@@ -438,10 +442,10 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                     Fx[P + 2] = xF[0 * LD + col + 1]; Fx[P + 3] = xF[1 * LD + col + 1];
 #pragma unroll
                     for (int p = 0; p < P; ++p) { Hx[2 + p] = H[p]; Fx[2 + p] = F[p]; }
-                    if (i0 == 0) {                           // x = 0: H even, F odd (R2)
+                    if (EDGE && i0 == 0) {                   // x = 0: H even, F odd (R2)
                         Hx[0] = Hx[4]; Hx[1] = Hx[3]; Fx[0] = -Fx[4]; Fx[1] = -Fx[3];
                     }
-                    if (any && i0 + P + 1 >= N - 1) {        // my window reaches i = N-1
+                    if (EDGE && any && i0 + P + 1 >= N - 1) {   // my window reaches i = N-1
                         const double lim = (16.0 * gE[2] - gE[3]) * K.inv12h2;   // F_{N-1} (R5)
 #pragma unroll
                         for (int k = 2; k < P + 4; ++k) {
@@ -463,11 +467,11 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                         const double dF = fma(8.0, Fx[p + 3] - Fx[p + 1], Fx[p] - Fx[p + 4]);
                         double vP = fma(K.d4c, dH, kP[p]);
                         double vQ = fma(tC8[p] * K.d4c, dF, kQ[p]);
-                        if (i == 0) {                        // eq (7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
+                        if (EDGE && i == 0) {                // eq (7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
                             vP = 0.0;
                             vQ = fma(8.0 * G1 - G2, K.c_org, kQ[p]);
                         }
-                        if (i >= N - 1) { vP = 0.0; vQ = 0.0; }                   // eqs (9), (10)
+                        if (EDGE && i >= N - 1) { vP = 0.0; vQ = 0.0; }           // eqs (9), (10)
                         // a5: RK combine
                         if (s == 0) {
                             ac0[p] = fma(b_w, vP, uP[3 + p]); ac1[p] = fma(b_w, vQ, uQ[3 + p]);
@@ -478,18 +482,18 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                         } else {
                             nP[p] = fma(b_w, vP, ac0[p]); nQ[p] = fma(b_w, vQ, ac1[p]);
                         }
-                        if (i > N - 1) { nP[p] = 0.0; nQ[p] = 0.0; ac0[p] = 0.0; ac1[p] = 0.0; }
+                        if (EDGE && i > N - 1) { nP[p] = 0.0; nQ[p] = 0.0; ac0[p] = 0.0; ac1[p] = 0.0; }
                     }
                     if (any) {
                         double *Sw = S + tl0 + tid;
 #pragma unroll
                         for (int p = 0; p < P; ++p) {
-                            if (l0 + p < cn) {
+                            if (!EDGE || l0 + p < cn) {
                                 Sw[p * T] = nP[p]; Sw[SP_CAP + p * T] = nQ[p]; Sw[2 * SP_CAP + p * T] = nA[p];
-                                if (i0 + p <= N - 2) {       // f' of the new stage state, for the next publish
+                                if (!EDGE || i0 + p <= N - 2) {   // f' of the new stage state, for the next publish
                                     const double f = m2sc[p] * fma(nP[p], nP[p], nQ[p] * nQ[p]);
                                     facc += f;
-                                    if (i0 + p == N - 2) misc[1] = f * (1.0 / 12.0);
+                                    if (EDGE && i0 + p == N - 2) misc[1] = f * (1.0 / 12.0);
                                 }
                             }
                         }
@@ -497,12 +501,19 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
                         double2 *d1 = reinterpret_cast<double2 *>((s < LS ? prm.ACC[1] : prm.U[1]) + row + i0);
 #pragma unroll
                         for (int p = 0; p < P; p += 2) {
-                            if (i0 + p >= pb.NP) continue;
+                            if (EDGE && i0 + p >= pb.NP) continue;
                             if (s < LS) { d0[p / 2] = make_double2(ac0[p], ac0[p + 1]); d1[p / 2] = make_double2(ac1[p], ac1[p + 1]); }
                             else { d0[p / 2] = make_double2(nP[p], nP[p + 1]); d1[p / 2] = make_double2(nQ[p], nQ[p + 1]); }
                         }
                     }
                     carry += ttot;
+                };   // tile_body
+                for (int tt = ntile - 1; tt >= 0; --tt) {
+                    // full tile, 8 points clear of x = 0 and of x = pi/2 (uniform over the CTA)
+                    const bool interior = (tt + 1) * S8_TILE <= cn && ci0 + tt * S8_TILE >= 8
+                                          && ci0 + (tt + 1) * S8_TILE + 8 <= N - 1;
+                    if (interior) tile_body(std::false_type{}, tt);
+                    else tile_body(std::true_type{}, tt);
                 }   // tiles
                 bad = __syncthreads_or(bad);
             }   // stages
@@ -520,14 +531,21 @@ __global__ void __launch_bounds__(S8_T, 1) k_stream_persist8(const __grid_consta
     }   // members
 }
 
-cudaError_t launch_stream_persist8(adsc_ctx *c, const SPParams &prm)
+template <int P_, int T_>
+static cudaError_t launch_shape(adsc_ctx *c, const SPParams &prm)
 {
-    cudaError_t e = cudaFuncSetAttribute((const void *)k_stream_persist8, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)S8Layout::bytes);
+    using L = S8Cfg<P_, T_>;
+    const void *fn = (const void *)k_stream_persist8<P_, T_>;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::bytes);
     if (e != cudaSuccess) return e;
     void *args[] = { (void *)&prm };
-    return cudaLaunchCooperativeKernel((const void *)k_stream_persist8, dim3((unsigned)(c->sp_G * c->sp_groups)),
-                                       dim3(S8_T), args, S8Layout::bytes, c->stream);
+    return cudaLaunchCooperativeKernel(fn, dim3((unsigned)(c->sp_G * c->sp_groups)), dim3(T_), args, L::bytes, c->stream);
+}
+
+// shape 8: 8 points x 224 threads (tiles of 1792); shape 84: 4 points x 256 threads (tiles of 1024)
+cudaError_t launch_stream_persist8(adsc_ctx *c, const SPParams &prm)
+{
+    return c->sp_ppt == 84 ? launch_shape<4, 256>(c, prm) : launch_shape<8, 224>(c, prm);
 }
 
 }  // namespace adsc
