@@ -42,7 +42,7 @@ N_SMS = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE stage-kernel launch from the committed `ncu --set full`
 # captures (profiles/r01_summary.md).  The state is loaded and stored once per launch whatever the number of
 # RK4 steps in it (resident path) or stays L2-resident (cfg4), so the figure does not scale with rk4_per_step.
-NCU_TRAFFIC_BYTES = {"cfg2": 148.4e6, "cfg5": 1562.0e6, "cfg3": 1563.0e6, "cfg4": 289.3e6, "cfg1": None}
+NCU_TRAFFIC_BYTES = {"cfg2": 148.4e6, "cfg5": 1562.0e6, "cfg3": 1563.0e6, "cfg4": 339.1e6, "cfg1": None}
 
 
 def parse():
