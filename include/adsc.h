@@ -68,7 +68,9 @@ extern "C" {
                                           streaming kernel: 4 (256 threads per CTA, 1024-point
                                           tiles; default), 2 (512 threads) or 8 (224 threads,
                                           1792-point tiles, register-blocked tile body) or 84 (that
-                                          tile body with 4 points x 256 threads); 8 and 84 have no
+                                          tile body with 4 points x 256 threads) or 42 (the default
+                                          body as TWO CTAs of 128 threads per SM, chunks of up to
+                                          3584 points); 8, 84 and 42 have no
                                           fixed-background build (4 is used instead).  Results do
                                           not depend on it beyond rounding order.               */
 

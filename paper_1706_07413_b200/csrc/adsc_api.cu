@@ -165,7 +165,7 @@ int adsc_set_option(adsc_handle h, int key, double value)
         if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
         return ADSC_OK;
     case ADSC_OPT_STREAM_PPT:
-        if (!(value == 2.0 || value == 4.0 || value == 8.0 || value == 84.0)) return fail(h, ADSC_EINVAL, "points per thread of the streaming kernel: 2, 4 or 8");
+        if (!(value == 2.0 || value == 4.0 || value == 8.0 || value == 84.0 || value == 42.0)) return fail(h, ADSC_EINVAL, "points per thread of the streaming kernel: 2, 4 or 8");
         h->sp_ppt = (int)value;
         return ADSC_OK;
     default:

@@ -21,18 +21,20 @@
 
 namespace adsc {
 
-constexpr int SP_TILE = 1024;                      // points per tile = threads x contiguous points per thread
-constexpr int SP_TILES = 7;                        // tiles per chunk
-static_assert(SP_CAP == SP_TILE * SP_TILES, "7168 points per CTA");
 constexpr int SP_HAL = 4;                          // lower halo slots of the chunk arrays (3 used)
 
 // Shared-memory index map: thread t touches P t + q (P = 2 or 4), a stride of P doubles; one padding
 // double per 16 makes those accesses conflict-free (16 consecutive lanes, 16 distinct 8-byte banks).
 __host__ __device__ constexpr int sp_pad(int j) { return j + (j >> 4); }
 
+// TILE = points per tile (threads x contiguous points per thread), CAP = points per CTA chunk: 7168 with one CTA
+// per SM, 3584 with two.
+template <int TILE, int CAP>
 struct SPLayout {
-    static constexpr int field = sp_pad(SP_CAP + SP_HAL + 4) + 1;   // one chunk array with lower halo
-    static constexpr int flux = sp_pad(SP_TILE + 4) + 1;            // tile + 2 halo points per side
+    static constexpr int SP_TILES = CAP / TILE;
+    static_assert(SP_TILES * TILE == CAP, "tiles must fill the chunk");
+    static constexpr int field = sp_pad(CAP + SP_HAL + 4) + 1;      // one chunk array with lower halo
+    static constexpr int flux = sp_pad(TILE + 4) + 1;               // tile + 2 halo points per side
     static constexpr int o_S = 0;                                   // [3][field]
     static constexpr int o_H = o_S + 3 * field;
     static constexpr int o_F = o_H + flux;
@@ -83,11 +85,13 @@ __device__ __forceinline__ double block_suffix_excl_sp(double S, double *sw, dou
 
 // FIXED: A = 1, delta = 0 held fixed (Table II): no f', no scan, E = 1, eq (4) not evolved, no
 // collapse test; the mailboxes then carry only the state edges.
-template <int P, int T, bool FIXED>
-__global__ void __launch_bounds__(T, 1) k_stream_persist(const __grid_constant__ SPParams prm)
+// CTAS: CTAs per SM (1: chunks of up to 7168 points; 2: chunks of up to 3584 points, two independent CTAs per SM).
+template <int P, int T, bool FIXED, int CTAS>
+__global__ void __launch_bounds__(T, CTAS) k_stream_persist(const __grid_constant__ SPParams prm)
 {
-    static_assert(P * T == SP_TILE && P >= 2, "a tile is 1024 points");
-    using L = SPLayout;
+    constexpr int SP_TILE = P * T;
+    static_assert(P >= 2 && (CTAS == 1 || CTAS == 2), "shape");
+    using L = SPLayout<SP_TILE, SP_CAP / CTAS>;
     extern __shared__ __align__(16) double smem[];
     double *S = smem + L::o_S, *sH = smem + L::o_H, *sF = smem + L::o_F, *up = smem + L::o_up;
     double *sw = smem + L::o_sw, *gE = smem + L::o_gE, *misc = smem + L::o_misc;
@@ -494,21 +498,22 @@ bool stream_persist_select(adsc_ctx *c)
 {
     c->sp_ok = false;
     if (c->dev_sms <= 0) return false;
-    const int N = c->pb.N, sms = c->dev_sms;
-    const int gmin = (N + SP_CAP - 1) / SP_CAP;
+    if (c->pb.fixed_bg && (c->sp_ppt == 8 || c->sp_ppt == 84 || c->sp_ppt == 42)) c->sp_ppt = 4;   // no fixed-background build
+    if (c->sp_ppt != 2 && c->sp_ppt != 4 && c->sp_ppt != 8 && c->sp_ppt != 84 && c->sp_ppt != 42) c->sp_ppt = 4;
+    const int ctas = (c->sp_ppt == 42) ? 2 : 1;                        // CTAs per SM
+    const int cap = SP_CAP / ctas, tile = (c->sp_ppt == 42) ? 512 : 1024;
+    const int N = c->pb.N, sms = c->dev_sms * ctas;                    // co-resident CTAs
+    const int gmin = (N + cap - 1) / cap;
     if (gmin > sms) return false;
-    const int per_member = sms / (c->pb.B < sms ? c->pb.B : sms);      // SMs a member can have
+    const int per_member = sms / (c->pb.B < sms ? c->pb.B : sms);      // CTAs a member can have
     int G = per_member;
-    const int gmax = (N + SP_TILE - 1) / SP_TILE;
+    const int gmax = (N + tile - 1) / tile;
     if (G > gmax) G = gmax;
     if (G < gmin) G = gmin;
-    if (c->pb.fixed_bg && c->sp_ppt == 8) c->sp_ppt = 4;     // the 8-point kernel has no fixed-background build
-    if ((c->pb.fixed_bg) && c->sp_ppt == 84) c->sp_ppt = 4;
-    if (c->sp_ppt != 2 && c->sp_ppt != 4 && c->sp_ppt != 8 && c->sp_ppt != 84) c->sp_ppt = 4;
     const int al = (c->sp_ppt == 8) ? 8 : 4;                 // chunks start on a thread boundary
     int Lc = ((N + G - 1) / G + al - 1) / al * al;
     G = (N + Lc - 1) / Lc;
-    if (Lc > SP_CAP || (G > 1 && N - (G - 1) * Lc < 8)) return false;
+    if (Lc > cap || (G > 1 && N - (G - 1) * Lc < 8)) return false;
     int groups = sms / G;
     if (groups > c->pb.B) groups = c->pb.B;
     if (groups < 1 || (size_t)groups * G > SP_MAX_CTAS) return false;
@@ -519,10 +524,16 @@ bool stream_persist_select(adsc_ctx *c)
 cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
 {
     const void *fn;
-    if (c->pb.fixed_bg) fn = c->sp_ppt == 4 ? (const void *)k_stream_persist<4, 256, true> : (const void *)k_stream_persist<2, 512, true>;
-    else fn = c->sp_ppt == 4 ? (const void *)k_stream_persist<4, 256, false> : (const void *)k_stream_persist<2, 512, false>;
-    const int threads = SP_TILE / c->sp_ppt;
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SPLayout::bytes);
+    int threads = 256;
+    size_t smem = SPLayout<1024, SP_CAP>::bytes;
+    if (c->pb.fixed_bg) {
+        if (c->sp_ppt == 2) { fn = (const void *)k_stream_persist<2, 512, true, 1>; threads = 512; }
+        else fn = (const void *)k_stream_persist<4, 256, true, 1>;
+    } else if (c->sp_ppt == 42) {
+        fn = (const void *)k_stream_persist<4, 128, false, 2>; threads = 128; smem = SPLayout<512, SP_CAP / 2>::bytes;
+    } else if (c->sp_ppt == 2) { fn = (const void *)k_stream_persist<2, 512, false, 1>; threads = 512; }
+    else fn = (const void *)k_stream_persist<4, 256, false, 1>;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(c->ws.sp_counter, 0, sizeof(unsigned long long) * SP_MAX_CTAS, c->stream);
     if (e != cudaSuccess) return e;
@@ -550,7 +561,7 @@ cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last)
     }
     void *args[] = { (void *)&prm };
     e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)(c->sp_G * c->sp_groups)), dim3((unsigned)threads), args,
-                                    SPLayout::bytes, c->stream);
+                                    smem, c->stream);
     c->launches++;
     return e;
 }

@@ -108,7 +108,7 @@ def test_config_shapes_1000_steps(env, name, B, path, nthr):
     assert np.max(np.abs(d["mass"] - od["mass"]) / np.abs(od["mass"])) <= 1e-11
 
 
-@pytest.mark.parametrize("path,ppt", [(1, 2), (1, 4), (1, 8), (1, 84), (3, None)])
+@pytest.mark.parametrize("path,ppt", [(1, 2), (1, 4), (1, 8), (1, 84), (1, 42), (3, None)])
 def test_streaming_many_tiles(env, path, ppt):
     """Streaming paths across many tiles with a ragged tail (N-1 not a tile multiple)."""
     N = 65 * 1024 + 137
@@ -141,7 +141,7 @@ def test_long_member_A_resolve_and_set_initial(env, path):
     assert (d["constraint_residual"] < 1e-12).all()
 
 
-@pytest.mark.parametrize("ppt", [4, 8, 84])
+@pytest.mark.parametrize("ppt", [4, 8, 84, 42])
 def test_streaming_more_members_than_groups(env, ppt):
     """Persistent streaming kernel with more members than concurrent groups: N=20481 needs 3 chunks
     per member, so 49 members run at once and the rest in a second round; N-1 = 4*5120 makes the
@@ -149,7 +149,7 @@ def test_streaming_more_members_than_groups(env, ppt):
     N, B = 20481, 60
     Phi, Pi, _ = env["inputs"].make("cfg5", B=B, N=N)
     ens, f, d = _gpu_run(env, Phi, Pi, 40, path=1, stream_ppt=ppt)
-    assert ens.path == (1, 3)
+    assert ens.path == (1, 6 if ppt == 42 else 3)
     ev = env["oracle"].Evolution(Phi, Pi, nthreads=8).step(40)
     _compare(f, ev)
     _bc_invariants(f)
@@ -170,7 +170,7 @@ def test_cfg4_full_size_sampled(env):
 @pytest.mark.parametrize("N,path,ppt", [(9, 1, 2), (17, 1, 4), (33, 1, 2), (129, 2, None), (1001, 1, 2), (257, 2, None),
                                         (513, 1, 4), (17, 3, None), (1001, 3, None), (1027, 1, 2), (1027, 1, 4),
                                         (2051, 1, 2), (2051, 1, 4), (9, 1, 8), (1027, 1, 8), (1793, 1, 8), (7177, 1, 8),
-                                        (1027, 1, 84), (7177, 1, 84)])
+                                        (1027, 1, 84), (7177, 1, 84), (1027, 1, 42), (7177, 1, 42)])
 def test_small_and_odd_sizes(env, N, path, ppt):
     rng = np.random.default_rng(7 + N)
     Phi, Pi, _ = env["inputs"].make("cfg5", B=5, N=N)
