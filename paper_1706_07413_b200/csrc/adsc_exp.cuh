@@ -49,15 +49,33 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P])
 {
     const double xr = x[P - 1];
     double z[P];
-    int big = 0;
+    int big = 0, mid = 0, sml = 0;
 #pragma unroll
     for (int p = 0; p < P - 1; ++p) {
         z[p] = x[p] - xr;
-        big |= ((__double2hiint(z[p]) & 0x7fffffff) > 0x3f900000) ? 1 : 0;    // |z| > 2^-6 (or NaN)
+        const int hz = __double2hiint(z[p]) & 0x7fffffff;
+        big |= (hz > 0x3f900000) ? 1 : 0;    // |z| > 2^-6 (or NaN)
+        mid |= (hz > 0x3f500000) ? 1 : 0;    // |z| > 2^-10
+        sml |= (hz > 0x3f100000) ? 1 : 0;    // |z| > 2^-14
     }
     const double Er = exp3_ref(xr);
     E[P - 1] = Er;
-    if (!big) {
+    if (!sml) {                              // |z| <= 2^-14: two terms of t suffice (z^4/24 < 6e-19)
+#pragma unroll
+        for (int p = 0; p < P - 1; ++p) {
+            double t = fma(z[p], c_exp[5], c_exp[4]);
+            t = fma(z[p], t, 1.0);
+            E[p] = fma(Er * z[p], t, Er);
+        }
+    } else if (!mid) {                       // |z| <= 2^-10: three terms of t suffice (z^5/120 < 8e-18)
+#pragma unroll
+        for (int p = 0; p < P - 1; ++p) {
+            double t = fma(z[p], c_exp[6], c_exp[5]);
+            t = fma(z[p], t, c_exp[4]);
+            t = fma(z[p], t, 1.0);
+            E[p] = fma(Er * z[p], t, Er);
+        }
+    } else if (!big) {
 #pragma unroll
         for (int p = 0; p < P - 1; ++p) {
             double t = fma(z[p], c_exp[8], c_exp[7]);
