@@ -55,7 +55,6 @@ def parse():
     ap.add_argument("--rk4-per-step", type=int, default=0, help="RK4 steps per bench step (0 = workload default)")
     ap.add_argument("--batch", type=int, default=0, help="override the ensemble size (0 = workload default)")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 persistent streaming, 2 resident, 3 generic streaming")
-    ap.add_argument("--variant", type=int, default=None, help="resident kernel variant (tuning; default auto)")
     ap.add_argument("--fixed-background", action="store_true",
                     help="time the fixed-background variant (A = 1, delta = 0 held fixed; PAPER.md:177 Table II)")
     ap.add_argument("--rk-order", type=int, default=4, choices=[2, 3, 4],
@@ -238,7 +237,7 @@ def main():
     Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all[lo:hi])).pin_memory()
     del Phi_all, Pi_all
 
-    ens = binding.Ensemble(N, B, device=dev, path=args.path, resident_variant=args.variant,
+    ens = binding.Ensemble(N, B, device=dev, path=args.path, 
                            fixed_background=args.fixed_background, rk_order=(args.rk_order if args.rk_order != 4 else None))
     path, cluster = ens.path
     Phi_d, Pi_d = Phi_h.to(dev), Pi_h.to(dev)
@@ -291,7 +290,7 @@ def main():
     # The user-facing way to run a batch from host memory: sub-batches on their own handles and streams, so that one
     # sub-batch's transfers overlap the other's kernels (binding.PipelinedEnsemble; members are independent).
     parts = max(1, min(args.e2e_parts, B // 32))
-    pe = binding.PipelinedEnsemble(N, B, parts=parts, device=dev, path=args.path, resident_variant=args.variant,
+    pe = binding.PipelinedEnsemble(N, B, parts=parts, device=dev, path=args.path, 
                                    fixed_background=args.fixed_background,
                                    rk_order=(args.rk_order if args.rk_order != 4 else None))
     for _ in range(1):

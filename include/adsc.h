@@ -49,30 +49,17 @@ extern "C" {
                                           A").  Default 0 = never.          */
 #define ADSC_OPT_PATH               3  /* 0 auto (default: resident if a member fits on
                                           chip, else streaming); 1 force the streaming path
-                                          (persistent kernel, stage state in shared memory,
-                                          u^n and accumulator in global memory; falls back
-                                          to 3 at adsc_bind if the member's CTAs cannot all
-                                          be co-resident); 2 force the resident
-                                          (shared-memory/register) kernel, EINVAL if it
-                                          cannot hold N; 3 force the generic streaming
-                                          kernels (one launch per phase, any N).        */
+                                          (persistent kernel: stage state in shared memory,
+                                          coefficient tables staged by bulk asynchronous
+                                          copies, u^n and accumulator in global memory; it
+                                          needs N-1 to be a multiple of 8 and all CTAs of a
+                                          member co-resident, and falls back to 3 otherwise);
+                                          2 force the resident (shared-memory/register)
+                                          kernel, EINVAL if it cannot hold N; 3 force the
+                                          generic streaming kernels (one launch per phase,
+                                          any N).                                        */
 #define ADSC_OPT_STEPS_PER_LAUNCH   4  /* resident path: RK4 steps per kernel launch
                                           (default 0 = all steps of a call in one launch) */
-
-#define ADSC_OPT_RESIDENT_VARIANT    5  /* tuning: -1 auto (default) or the index of the one
-                                          resident kernel configuration (points per thread x
-                                          threads per CTA) to use; EINVAL if it cannot tile N.
-                                          Results do not depend on it beyond rounding order.  */
-
-#define ADSC_OPT_STREAM_PPT          6  /* tuning: contiguous points per thread of the persistent
-                                          streaming kernel: 4 (256 threads per CTA, 1024-point
-                                          tiles; default), 2 (512 threads) or 8 (224 threads,
-                                          1792-point tiles, register-blocked tile body) or 84 (that
-                                          tile body with 4 points x 256 threads) or 42 (the default
-                                          body as TWO CTAs of 128 threads per SM, chunks of up to
-                                          3584 points); 8, 84 and 42 have no
-                                          fixed-background build (4 is used instead).  Results do
-                                          not depend on it beyond rounding order.               */
 
 #define ADSC_OPT_FIXED_BACKGROUND    7  /* 1: evolve on the fixed background A = 1, delta = 0 (the
                                           paper's second workload, Table II): the
@@ -112,7 +99,9 @@ typedef struct {
  *   courant  dt = courant*h, 0 < courant <= 1 (method-of-lines RK4)
  *   ko_eps   >= 0: Kreiss-Oliger coefficient of the 7-point dissipation added to the
  *            right-hand sides of Phi and Pi (BASELINE.json configs[0]; not in the paper)
- * Host-only; touches no device.  Returns NULL on bad arguments or host OOM. */
+ * Host-only: launches nothing and allocates nothing on a device (it only asks the CUDA runtime for the SM count
+ * of the current device, if there is one, to size the streaming layout).  Returns NULL on bad arguments or host
+ * OOM; the message is kept per calling thread for adsc_last_error(NULL). */
 adsc_handle adsc_create(int N, int batch, double courant, double ko_eps);
 
 /* Release the handle (not the workspace).  NULL is allowed. */

@@ -20,8 +20,6 @@ ADSC_OPT_COLLAPSE_THRESHOLD = 1
 ADSC_OPT_A_RESOLVE_PERIOD = 2
 ADSC_OPT_PATH = 3
 ADSC_OPT_STEPS_PER_LAUNCH = 4
-ADSC_OPT_RESIDENT_VARIANT = 5
-ADSC_OPT_STREAM_PPT = 6
 ADSC_OPT_FIXED_BACKGROUND = 7
 ADSC_OPT_RK_ORDER = 8
 PATH_AUTO, PATH_STREAM, PATH_RESIDENT = 0, 1, 2
@@ -175,7 +173,7 @@ class Ensemble:
 
     def __init__(self, N, batch, courant=0.25, ko_eps=0.1, device="cuda:0", stream=None,
                  path=PATH_AUTO, threshold=None, a_resolve_period=None, steps_per_launch=None,
-                 resident_variant=None, stream_ppt=None, fixed_background=False, rk_order=None):
+                 fixed_background=False, rk_order=None):
         import torch
         load_library()
         if not torch.cuda.is_available():
@@ -197,10 +195,6 @@ class Ensemble:
                 adsc_set_option(self.h, ADSC_OPT_A_RESOLVE_PERIOD, a_resolve_period)
             if steps_per_launch is not None:
                 adsc_set_option(self.h, ADSC_OPT_STEPS_PER_LAUNCH, steps_per_launch)
-            if resident_variant is not None:
-                adsc_set_option(self.h, ADSC_OPT_RESIDENT_VARIANT, resident_variant)
-            if stream_ppt is not None:
-                adsc_set_option(self.h, ADSC_OPT_STREAM_PPT, stream_ppt)
             with torch.cuda.device(self.device):
                 self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
                 nbytes = adsc_workspace_bytes(self.h)

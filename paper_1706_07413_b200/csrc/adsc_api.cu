@@ -10,7 +10,7 @@
 
 using namespace adsc;
 
-static std::string g_create_error = "";
+static thread_local std::string g_create_error = "";   // per calling thread: adsc_create has no handle to hang it on
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -36,19 +36,34 @@ static void compute_layout(adsc_ctx *c)
     L.off_part = off; off += stream ? 6 * tiles : 0;
     for (int k = 0; k < 2; ++k) { L.off_stage[k] = off; off += ext; }
     L.off_tab = off; off += align_up((size_t)5 * (c->pb.NP + 2 * HAL) * sizeof(double), 256);
+    L.off_tabp = off; off += (c->path == 1) ? align_up((size_t)3 * c->pb.NP * sizeof(double), 256) : 0;
     L.off_rec = off; off += align_up((size_t)c->pb.B * sizeof(MemberRec), 256);
     L.off_mbox = off; off += align_up((size_t)SP_MAX_CTAS * 2 * 24 * sizeof(double), 256);
     L.off_cnt = off; off += align_up((size_t)SP_MAX_CTAS * sizeof(unsigned long long), 256);
     L.total = off;
 }
 
+// Row pitch of the persistent streaming layout: G chunks of SQ 256-point slices hold the points 0..N-2; the row must
+// also hold the point N-1, so one more slice is added when the chunks end exactly there.
+static int sa_row_pitch(int N, int G, int SQ)
+{
+    const int np = G * SQ * 256;
+    return np >= N ? np : np + 256;
+}
+
+// Which kernel family steps this handle, and the internal row pitch NP that goes with it: rows are padded to a
+// multiple of 4 points, except on the persistent streaming path, whose rows are G chunks of SQ 256-point slices.
 static void resolve_path(adsc_ctx *c)
 {
     const bool can_res = resident_select(c);
-    if (c->path_opt == 1 || c->path_opt == 3) c->path = c->path_opt;
+    const bool can_sa = stream_async_select(c->pb.N, c->pb.B, c->sms_hint, &c->sp_G, &c->sp_SQ, &c->sp_groups);
+    c->sp_ok = can_sa;
+    if (c->path_opt == 3) c->path = 3;
+    else if (c->path_opt == 1) c->path = can_sa ? 1 : 3;
     else if (c->path_opt == 2) c->path = can_res ? 2 : 0;
-    else c->path = can_res ? 2 : 1;
+    else c->path = can_res ? 2 : (can_sa ? 1 : 3);
     if (c->path != 2) c->cluster = 1;
+    c->pb.NP = (c->path == 1) ? sa_row_pitch(c->pb.N, c->sp_G, c->sp_SQ) : (c->pb.N + 3) / 4 * 4;
     compute_layout(c);
 }
 
@@ -80,7 +95,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     if ((double)N * (double)batch > 4.0e9) { g_create_error = "N*batch too large"; return nullptr; }
     adsc_ctx *c = new (std::nothrow) adsc_ctx();
     if (!c) { g_create_error = "host allocation failed"; return nullptr; }
-    c->pb.N = N; c->pb.NP = (N + 3) / 4 * 4; c->pb.B = batch;
+    c->pb.N = N; c->pb.NP = (N + 3) / 4 * 4; c->pb.B = batch;   // (NP is final after resolve_path)
     c->pb.h = 1.5707963267948966192313216916398 / (double)(N - 1);
     c->courant = courant;
     c->pb.dt = courant * c->pb.h;
@@ -91,8 +106,18 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->K_A = 0; c->path_opt = 0; c->steps_per_launch = 0;
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
-    c->cluster = 1; c->res_cfg = -1; c->res_force = -1;
-    c->sp_ok = false; c->sp_G = 0; c->sp_groups = 0; c->sp_Lc = 0; c->sp_ppt = 4;
+    c->cluster = 1; c->res_cfg = -1;
+    c->sp_ok = false; c->sp_G = 0; c->sp_groups = 0; c->sp_SQ = 0;
+    // The row pitch of the persistent streaming path depends on the SM count.  adsc_create touches no device state;
+    // it only asks the runtime how many SMs the current device has, and assumes a B200 (148) if there is none to ask.
+    c->sms_hint = 148;
+    {
+        int ndev = 0, dev = 0, sms = 0;
+        if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0 && cudaGetDevice(&dev) == cudaSuccess
+            && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            c->sms_hint = sms;
+        else (void)cudaGetLastError();
+    }
     resolve_path(c);
     return c;
 }
@@ -138,18 +163,6 @@ int adsc_set_option(adsc_handle h, int key, double value)
         if (!(value >= 0.0) || value != std::floor(value)) return fail(h, ADSC_EINVAL, "steps per launch must be a non-negative integer");
         h->steps_per_launch = (long long)value;
         return ADSC_OK;
-    case ADSC_OPT_RESIDENT_VARIANT: {
-        if (value != std::floor(value) || value < -1.0 || value > 64.0) return fail(h, ADSC_EINVAL, "bad resident variant");
-        if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_RESIDENT_VARIANT before adsc_bind");
-        const int old = h->res_force;
-        h->res_force = (int)value;
-        resolve_path(h);
-        if (h->path != 2) {
-            h->res_force = old; resolve_path(h);
-            return fail(h, ADSC_EINVAL, "this resident variant cannot hold N (or the path is forced to streaming)");
-        }
-        return ADSC_OK;
-    }
     case ADSC_OPT_FIXED_BACKGROUND:
         if (!(value == 0.0 || value == 1.0)) return fail(h, ADSC_EINVAL, "fixed background: 0 or 1");
         if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_FIXED_BACKGROUND before adsc_bind");
@@ -163,10 +176,6 @@ int adsc_set_option(adsc_handle h, int key, double value)
         h->rk_order = (int)value;
         resolve_path(h);                 // (generation-1 and tuning configurations of the resident kernel are RK4 only)
         if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
-        return ADSC_OK;
-    case ADSC_OPT_STREAM_PPT:
-        if (!(value == 2.0 || value == 4.0 || value == 8.0 || value == 84.0 || value == 42.0)) return fail(h, ADSC_EINVAL, "points per thread of the streaming kernel: 2, 4 or 8");
-        h->sp_ppt = (int)value;
         return ADSC_OK;
     default:
         return fail(h, ADSC_EINVAL, "unknown option key");
@@ -209,8 +218,14 @@ int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream)
     h->ws.rec = (MemberRec *)(base + L.off_rec);
     h->ws.sp_mbox = (double *)(base + L.off_mbox);
     h->ws.sp_counter = (unsigned long long *)(base + L.off_cnt);
-    // the persistent streaming kernel needs every CTA of a member co-resident; otherwise one kernel per phase
-    if (h->path == 1 && !stream_persist_select(h)) h->path = 3;
+    h->ws.tabp = (double *)(base + L.off_tabp);
+    // the persistent streaming kernel needs every CTA of a member co-resident on THIS device and the row pitch the
+    // layout was made for; otherwise one kernel per phase (which takes any pitch)
+    if (h->path == 1) {
+        int G = 0, SQ = 0, groups = 0;
+        if (!stream_async_select(h->pb.N, h->pb.B, h->dev_sms, &G, &SQ, &groups) || sa_row_pitch(h->pb.N, G, SQ) != h->pb.NP) { h->path = 3; h->sp_ok = false; }
+        else { h->sp_G = G; h->sp_SQ = SQ; h->sp_groups = groups; }
+    }
     const size_t NT = (size_t)h->pb.NP + 2 * HAL;
     h->tb.sc = h->ws.tab + 0 * NT + HAL;
     h->tb.T = h->ws.tab + 1 * NT + HAL;
@@ -221,6 +236,7 @@ int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream)
     h->have_state = false;
     h->bound = true;
     ADSC_CUDA(launch_tables(h), "tables kernel");
+    if (h->path == 1) ADSC_CUDA(launch_tabp(h), "permuted tables kernel");
     return ADSC_OK;
 }
 
@@ -280,7 +296,7 @@ int adsc_step(adsc_handle h, long long nsteps)
             if (h->steps_per_launch > 0 && n > h->steps_per_launch) n = h->steps_per_launch;
             const bool hit = K > 0 && ((h->global_step + n) % K == 0);
             if (h->path == 2) ADSC_CUDA(launch_resident(h, n, hit ? 0 : 1), "resident kernel");
-            else ADSC_CUDA(launch_stream_persist(h, n, hit ? 0 : 1), "persistent streaming kernel");
+            else ADSC_CUDA(launch_stream_async(h, n, hit ? 0 : 1), "persistent streaming kernel");
             if (hit) {
                 ADSC_CUDA(launch_solve(h, SOLVE_WRITE_A | SOLVE_ACTIVE_ONLY), "A re-solve");
                 ADSC_CUDA(launch_finalize(h, 0), "finalize");

@@ -47,7 +47,7 @@ struct Problem {
 // Device pointers into the caller's workspace.
 struct Workspace {
     double *U[3];        // state Phi, Pi, A          [B][NP]
-    double *Ua[3];       // streaming: stage state ping
+    double *Ua[3];       // generic streaming: stage state ping; persistent streaming: u^n in the permuted layout
     double *Ub[3];       // streaming: stage state pong
     double *ACC[3];      // streaming: u^n + dt/6 * partial sum
     double *dl;          // streaming: tile-local suffix sums of I; also delta scratch
@@ -60,12 +60,13 @@ struct Workspace {
     double *sp_mbox;     // persistent streaming: [SP_MAX_CTAS][2][24] chunk mailboxes
     unsigned long long *sp_counter;   // persistent streaming: [SP_MAX_CTAS] group barrier counters
     double *tab;         // 5 tables
+    double *tabp;        // persistent streaming: -2 sc, tan^2, cot^2/(12h) permuted per 256-point slice [NP/256][3][256]
     MemberRec *rec;      // [B]
 };
 
 struct Layout {
     size_t off_U[3], off_Ua[3], off_Ub[3], off_ACC[3], off_dl, off_Ac, off_tot, off_carry, off_tot2, off_carry2, off_part,
-        off_stage[2], off_tab, off_rec, off_mbox, off_cnt, total;
+        off_stage[2], off_tab, off_tabp, off_rec, off_mbox, off_cnt, total;
     int ntiles;
 };
 
@@ -80,7 +81,6 @@ struct adsc_ctx {
     int path;                // resolved: 1 streaming (persistent), 2 resident, 3 streaming (one kernel per phase)
     int cluster;             // CTAs per member (resident)
     int res_cfg;             // index into the resident configuration table
-    int res_force;           // ADSC_OPT_RESIDENT_VARIANT: -1 auto, else the only table entry tried
     bool bound, have_state;
     cudaStream_t stream;
     void *ws_base;
@@ -92,9 +92,9 @@ struct adsc_ctx {
     int dev_sms;
     int dev_smem_optin;
     bool sp_ok;              // persistent streaming kernel usable (decided at adsc_bind)
-    int sp_G, sp_groups, sp_Lc;   // chunks per member, concurrent members, points per chunk
+    int sp_G, sp_groups, sp_SQ;   // chunks per member, concurrent members, 256-point slices per chunk
+    int sms_hint;            // SM count assumed for the layout (the device's if one was visible at adsc_create, else 148)
     int rk_order;            // 4 (classical RK4, default), 3 (Heun's third-order rule) or 2 (explicit midpoint): R12, R25
-    int sp_ppt;              // points per thread of the persistent streaming kernel: 2 (512 threads) or 4 (256)
     std::string err;
 };
 
@@ -126,8 +126,10 @@ constexpr int SOLVE_TILED_MIN_N = 32768;                      // members at leas
 cudaError_t launch_finalize(adsc_ctx *c, int inc_steps);
 cudaError_t launch_mode_energies(adsc_ctx *c, int J, double *d_out);   // adsc_modes.cu; d_out [B][J]
 cudaError_t launch_stream_step(adsc_ctx *c);                 // one RK4 step, generic streaming kernels
-bool stream_persist_select(adsc_ctx *c);                     // fills c->sp_* (needs c->dev_sms)
-cudaError_t launch_stream_persist(adsc_ctx *c, long long nsteps, int check_last);   // persistent streaming kernel
+// persistent streaming kernel (adsc_stream_async.cu): chunks per member, slices per chunk, concurrent members
+bool stream_async_select(int N, int B, int sms, int *G, int *SQ, int *groups);
+cudaError_t launch_tabp(adsc_ctx *c);                        // permuted coefficient tables for its bulk copies
+cudaError_t launch_stream_async(adsc_ctx *c, long long nsteps, int check_last);
 cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last);  // resident path
 bool resident_select(adsc_ctx *c);                           // fills c->cluster, c->res_cfg
 const char *resident_cfg_name(int cfg);

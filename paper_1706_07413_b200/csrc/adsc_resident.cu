@@ -381,7 +381,6 @@ bool resident_select(adsc_ctx *c)
     const int n_act = c->pb.N - 1;
     for (int k = 0; k < n_cfgs(); ++k) {
         const ResConfig &g = cfg_at(k);
-        if (c->res_force >= 0 && c->res_force != k) continue;
         if (n_act % g.seg) continue;
         const int cl = n_act / g.seg;
         if (cl < 1 || cl > 8) continue;

@@ -29,6 +29,7 @@
 #include "adsc_internal.cuh"
 #include "adsc_resident.cuh"
 #include "adsc_exp.cuh"
+#include "adsc_ptx.cuh"
 
 namespace adsc {
 
@@ -54,56 +55,6 @@ struct Res3Layout {
     static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
     static_assert(o_wt % 2 == 0, "warp-total slots must be 16-byte aligned");
 };
-
-// ---- mbarrier / cluster primitives (PTX; sm_90+)
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ uint32_t cluster_rank()
-{
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ uint32_t map_rank(uint32_t addr, int rank)
-{
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ void mbar_init(uint32_t mb, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mb), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t mb)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(mb) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t mb, uint32_t bytes)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(mb), "r"(bytes) : "memory");
-}
-template <bool CLUSTER_SCOPE>
-__device__ __forceinline__ void mbar_wait(uint32_t mb, uint32_t parity)
-{
-    if (CLUSTER_SCOPE)
-        asm volatile("{\n\t.reg .pred p;\n\tLAB_WAIT:\n\t"
-                     "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
-                     "@p bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(mb), "r"(parity) : "memory");
-    else
-        asm volatile("{\n\t.reg .pred p;\n\tLAB_WAIT:\n\t"
-                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-                     "@p bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(mb), "r"(parity) : "memory");
-}
-// Remote store into a peer CTA's shared memory that completes 8 (16) transaction bytes on the peer's mbarrier.
-__device__ __forceinline__ void st_async_f64(uint32_t dst_cluster, double v, uint32_t mbar_cluster)
-{
-    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];"
-                 ::"r"(dst_cluster), "l"(__double_as_longlong(v)), "r"(mbar_cluster) : "memory");
-}
-__device__ __forceinline__ void st_async_f64x2(uint32_t dst_cluster, double v0, double v1, uint32_t mbar_cluster)
-{
-    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];"
-                 ::"r"(dst_cluster), "l"(__double_as_longlong(v0)), "l"(__double_as_longlong(v1)), "r"(mbar_cluster) : "memory");
-}
 
 // FIXED: the paper's second workload (Table II), A = 1 and delta = 0 held fixed: no f', no scan,
 // no exponential, eq (4) not evolved, no collapse test -- the same stencils, exchanges and RK combine.
