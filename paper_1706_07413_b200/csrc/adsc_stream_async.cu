@@ -29,6 +29,9 @@
 #include "adsc_internal.cuh"
 #include "adsc_exp.cuh"
 #include "adsc_ptx.cuh"
+#ifdef SA_DEBUG
+#include <cstdio>
+#endif
 
 namespace adsc {
 
@@ -85,6 +88,7 @@ struct SAParams {
     long long nsteps;
     int check_last;
     int G, groups, SQ;               // chunks per member, concurrent members, slices per chunk
+    unsigned zero;                   // 0, but unknown to the compiler (see ring_next)
     SAConsts k;
 };
 
@@ -153,10 +157,8 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     const bool phys_lo = (c == 0), phys_hi = (c == G - 1);
     const int t_last = npts / P - 1;                     // chunk-level index of the thread that owns the last point
     const int cs0 = c * prm.SQ;                          // first slice of the chunk within a member row
-    unsigned long long *cnt = prm.counter + gi;
-    double *mb = prm.mbox + (size_t)gi * 2 * G * SA_MBOX;
-    unsigned long long epoch = 0;
-    unsigned stage_ctr = 0;                              // runs on across members: mailbox parity never repeats early
+    unsigned stage_ctr = 0;                              // barrier rounds so far; runs on across members, so the
+                                                         // mailbox parity never repeats early
 
     const uint32_t mbF = smem_u32(misc + o_mbar);
     const uint32_t mbR = mbF + 8 + (uint32_t)warp * 24;  // this warp's three ring barriers
@@ -167,6 +169,8 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
         for (int k = 0; k < 3 * SA_NW; ++k) mbar_init(mbF + 8 + 8 * k, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    // columns of threads that own no point are read as halos by their neighbours: keep them finite
+    for (int k = tid; k < 3 * SA_FS; k += SA_T) S[k] = make_double2(0.0, 0.0);
     // tables around the boundaries the pre-pass serves (chunk bottom, tile bottoms, chunk top) and at slice edges
     if (tid < 30) {
         const int m = tid / 6, k = tid - 6 * m;
@@ -189,31 +193,27 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     // keeps its tables for the whole launch.
     unsigned rpar = 0;                                   // phase parity per slot
     const bool reload = n_my > 1;
-    auto ring_issue = [&](int t, int qn) {
+    auto ring_issue = [&](int t, int qn, unsigned dep) {
         if (lane == 0) {
-            const uint32_t mbt = mbR + 8 * t;
-            mbar_arrive_expect_tx(mbt, SA_SLOT);
-            bulk_g2s(ringw + t * SA_SLOT, prm.tabp + ((size_t)(cs0 + qn) * 3 + t) * SA_SL, SA_SLOT, mbt);
+            bulk_g2s_after_reads(ringw + t * SA_SLOT, prm.tabp + ((size_t)(cs0 + qn) * 3 + t) * SA_SL,
+                                 SA_SLOT + (dep & prm.zero), mbR + 8 * t);
         }
     };
-    int pending = 0;                                     // slots with a copy in flight that nobody has waited for
     if (n_my > 0) {
         const int q0 = SA_NW * (n_my - 1) + warp;
-        if (!FIXED) ring_issue(0, q0);
-        ring_issue(1, q0); ring_issue(2, q0);
-        pending = FIXED ? 6 : 7;
+        if (!FIXED) ring_issue(0, q0, 0u);
+        ring_issue(1, q0, 0u); ring_issue(2, q0, 0u);
     }
-    auto ring_wait = [&](int t) {
-        mbar_wait<false>(mbR + 8 * t, (rpar >> t) & 1u);
-        pending &= ~(1 << t);
-    };
-    // after the warp has read slot t of slice q (tile j): fetch the same table of its next slice
-    auto ring_next = [&](int t, int j) {
+    auto ring_wait = [&](int t) { mbar_wait<false>(mbR + 8 * t, (rpar >> t) & 1u); };
+    // After the warp has read slot t of slice q (tile j): fetch the same table of its next slice.  The copy engine is
+    // not ordered behind the warp's shared-memory loads, so the copy is made to DEPEND on them: `dep` mixes one word of
+    // every load of the slot into the byte count (and with a run-time zero), and the copy is predicated on the state
+    // token of the mbarrier arrive (adsc_ptx.cuh).  Without this a queued load could read the NEXT slice's table.
+    auto ring_next = [&](int t, int j, unsigned dep) {
         if (reload) {
-            __syncwarp();
-            ring_issue(t, SA_NW * (j > 0 ? j - 1 : n_my - 1) + warp);
+            dep = __reduce_or_sync(FULL, dep);
+            ring_issue(t, SA_NW * (j > 0 ? j - 1 : n_my - 1) + warp, dep);
             rpar ^= 1u << t;
-            pending |= 1 << t;
         }
     };
 
@@ -230,7 +230,6 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
         const size_t prow = row + (size_t)ci0;                       // the chunk in the permuted arrays
 
         // ---- load the chunk: natural layout -> shared memory (stage state) and the permuted u^n; slice totals
-        double ex0 = 0.0, ex1 = 0.0, ex2 = 0.0, ex3 = 0.0;           // exclusive warp-level suffix of f' per tile
         for (int j = 0; j < n_my; ++j) {
             const int q = SA_NW * j + warp, l0 = q * SA_SL + lane * P;
             const int R = sa_rs(j);
@@ -268,8 +267,6 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                 }
                 if (phys_hi && (l0 >> 3) == t_last) tot += f7 * (1.0 / 12.0);    // top term of the telescoped rule
                 const double incl = warp_suffix_incl(tot);
-                const double ex = incl - tot;
-                if (j == 0) ex0 = ex; else if (j == 1) ex1 = ex; else if (j == 2) ex2 = ex; else ex3 = ex;
                 if (lane == 0) { wt[q] = incl; wfl[q] = 0.0; }
             }
         }
@@ -283,6 +280,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                 __syncthreads();                                         // S1: state, slice totals, flags of every tile
                 if (warp == 0) {
                     // ---- a2, slice level: exclusive suffix over the chunk's slices; chunk total and edges to the mailbox
+                    double *mb = prm.mbox + (size_t)gi * 2 * G * SA_MBOX;
                     double *mine = mb + ((size_t)par * G + c) * SA_MBOX;
                     double exq = 0.0;
                     if constexpr (!FIXED) {
@@ -301,13 +299,14 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     __threadfence();
                     __syncwarp();
                     if (lane == 0) {
-                        const unsigned long long target = (++epoch) * (unsigned long long)G;
+                        unsigned long long *cnt = prm.counter + gi;
+                        const unsigned long long target = (unsigned long long)stage_ctr * (unsigned long long)G;
                         atomicAdd(cnt, 1ULL);
                         unsigned long long v;
                         do {
                             asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(cnt) : "memory");
                         } while (v < target);
-                    } else ++epoch;
+                    }
                     __syncwarp();
                     // ---- gather: totals of the chunks above, flags, neighbour edges / parity ghosts
                     const double *all = mb + (size_t)par * G * SA_MBOX;
@@ -423,13 +422,11 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     const size_t po = prow + (size_t)q * SA_SL + lane * 4;
 
                     // ------------------------------------------------------------ phase 1
-                    double ph[P], pi[P], a[P];
+                    double ph[P], pi[P];
 #pragma unroll
                     for (int k = 0; k < 4; ++k) {
                         const double2 x = sP[k * R], y = sP[SA_FS + k * R];
                         ph[2 * k] = x.x; ph[2 * k + 1] = x.y; pi[2 * k] = y.x; pi[2 * k + 1] = y.y;
-                        if constexpr (!FIXED) { const double2 z = sP[2 * SA_FS + k * R]; a[2 * k] = z.x; a[2 * k + 1] = z.y; }
-                        else { a[2 * k] = 1.0; a[2 * k + 1] = 1.0; }
                     }
                     double hlP[3], hrP[3], hlQ[3], hrQ[3];                // 3 halo points per side of the stage state
                     {
@@ -442,18 +439,6 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         const double2 v0 = h0[0], v1 = h1[0], y0 = h0[foh], y1 = h1[foh];
                         hrP[0] = v0.x; hrP[1] = v0.y; hrP[2] = v1.x; hrQ[0] = y0.x; hrQ[1] = y0.y; hrQ[2] = y1.x;
                     }
-                    // global operands of the A update (needed at the end of phase 1): issued first
-                    double unA[P], acA[P];
-                    if constexpr (!FIXED) {
-                        if (s > 0) {
-                            ldg256(prm.ACC[2] + po, acA[0], acA[1], acA[2], acA[3]);
-                            ldg256(prm.ACC[2] + po + 128, acA[4], acA[5], acA[6], acA[7]);
-                            if (s < LS) {
-                                ldg256(prm.UN[2] + po, unA[0], unA[1], unA[2], unA[3]);
-                                ldg256(prm.UN[2] + po + 128, unA[4], unA[5], unA[6], unA[7]);
-                            }
-                        }
-                    }
                     double m2[P], fm = 0.0, fp = 0.0;
                     if constexpr (FIXED) {
 #pragma unroll
@@ -464,7 +449,8 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         for (int k = 0; k < 4; ++k) { const double2 m = slot[k * 32 + lane]; m2[2 * k] = m.x; m2[2 * k + 1] = m.y; }
                         const double scm = (lane == 0) ? esc[2 * q] : slot[3 * 32 + lane - 1].y;
                         const double scp = (lane == 31) ? esc[2 * q + 1] : slot[lane + 1].x;
-                        ring_next(0, j);
+                        ring_next(0, j, (unsigned)(__double2hiint(m2[0]) | __double2hiint(m2[2]) | __double2hiint(m2[4]) | __double2hiint(m2[6])
+                                                   | __double2hiint(scm) | __double2hiint(scp)));
                         fm = scm * fma(hlP[2], hlP[2], hlQ[2] * hlQ[2]);          // f'_{-1}
                         fp = scp * fma(hrP[0], hrP[0], hrQ[0] * hrQ[0]);          // f'_{P}
                     }
@@ -495,8 +481,9 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         so[P - 1] = fo[P - 1] + top;
 #pragma unroll
                         for (int p = P - 2; p >= 0; --p) so[p] = so[p + 1] + fo[p];
-                        const double ex = (j == 0) ? ex0 : (j == 1) ? ex1 : (j == 2) ? ex2 : ex3;
-                        const double B = ex + base[q];
+                        // a2, warp level: exclusive suffix over the lanes (the shuffle chain overlaps the arithmetic around it)
+                        const double st = live ? so[0] : 0.0;             // (dead lanes may hold anything)
+                        const double B = warp_suffix_incl(st) - st + base[q];
                         // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f
                         double nd[P];
 #pragma unroll
@@ -510,15 +497,39 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             nd[p] = fma(K.hh, s2 + B, loc);
                         }
                         exp3_near<P>(nd, E);
+#ifdef SA_DEBUG
+                        if (blockIdx.x == 0 && warp == 0 && lane < 4 && n == 0) printf("s%d lane%d B=%g base=%g so0=%g fm=%g fp=%g nd0=%g nd7=%g E0=%g E7=%g ph0=%g ph7=%g m2_0=%g m2_7=%g hlP=%g %g %g hrP=%g %g %g\n", s, lane, B, base[q], so[0], fm, fp, nd[0], nd[7], E[0], E[7], ph[0], ph[7], m2[0], m2[7], hlP[0], hlP[1], hlP[2], hrP[0], hrP[1], hrP[2]);
+#endif
+                    }
+                    // global operands of the A update (needed at the end of phase 1)
+                    double unA[P], acA[P];
+                    if constexpr (!FIXED) {
+                        if (s > 0) {
+                            ldg256(prm.ACC[2] + po, acA[0], acA[1], acA[2], acA[3]);
+                            ldg256(prm.ACC[2] + po + 128, acA[4], acA[5], acA[6], acA[7]);
+                            if (s < LS) {
+                                ldg256(prm.UN[2] + po, unA[0], unA[1], unA[2], unA[3]);
+                                ldg256(prm.UN[2] + po + 128, unA[4], unA[5], unA[6], unA[7]);
+                            }
+                        }
                     }
                     // a3 fluxes
-                    double H[P], F[P], kAv[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
+                    double H[P], F[P], kAv[P], a[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
                     {
                         ring_wait(1);
                         double tT[P];
 #pragma unroll
                         for (int k = 0; k < 4; ++k) { const double2 m = slot[128 + k * 32 + lane]; tT[2 * k] = m.x; tT[2 * k + 1] = m.y; }
-                        ring_next(1, j);
+                        ring_next(1, j, (unsigned)(__double2hiint(tT[0]) | __double2hiint(tT[2]) | __double2hiint(tT[4]) | __double2hiint(tT[6])));
+                        // the stage state is read again (it is still unchanged in shared memory) rather than kept in
+                        // registers across the exponentials
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const double2 x = sP[k * R], y = sP[SA_FS + k * R];
+                            ph[2 * k] = x.x; ph[2 * k + 1] = x.y; pi[2 * k] = y.x; pi[2 * k + 1] = y.y;
+                            if constexpr (!FIXED) { const double2 z = sP[2 * SA_FS + k * R]; a[2 * k] = z.x; a[2 * k + 1] = z.y; }
+                            else { a[2 * k] = 1.0; a[2 * k + 1] = 1.0; }
+                        }
 #pragma unroll
                         for (int p = 0; p < P; ++p) {
                             const double AE = a[p] * E[p];
@@ -586,11 +597,17 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     warp_arrive(mbF);                                             // sync F: arrive
 
                     // ------------------------------------------------------------ between arrive and wait
-                    double dH[P], dF[P];
+                    // a4 for the interior points p in [2, P-2), which need own fluxes only: their differences go
+                    // straight into the right-hand sides, in the shadow of the slowest warp's arrival
+                    double tC[P];
+                    ring_wait(2);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { const double2 m = slot[256 + k * 32 + lane]; tC[2 * k] = m.x; tC[2 * k + 1] = m.y; }
+                    ring_next(2, j, (unsigned)(__double2hiint(tC[0]) | __double2hiint(tC[2]) | __double2hiint(tC[4]) | __double2hiint(tC[6])));
 #pragma unroll
                     for (int p = 2; p < P - 2; ++p) {
-                        dH[p] = fma(8.0, H[p + 1] - H[p - 1], H[p - 2] - H[p + 2]);
-                        dF[p] = fma(8.0, F[p + 1] - F[p - 1], F[p - 2] - F[p + 2]);
+                        kP[p] = fma(K.d4c, fma(8.0, H[p + 1] - H[p - 1], H[p - 2] - H[p + 2]), kP[p]);
+                        kQ[p] = fma(tC[p], fma(8.0, F[p + 1] - F[p - 1], F[p - 2] - F[p + 2]), kQ[p]);
                     }
                     mbar_wait<false>(mbF, fpar);                                  // sync F: wait
 
@@ -610,29 +627,19 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         Hp0 = 0.0; Hp1 = -H[P - 1];
                         Fp0 = (16.0 * Gl1 - Gl2) * K.inv12h2; Fp1 = F[P - 1];
                     }
-                    dH[0] = fma(8.0, H[1] - Hm1, Hm2 - H[2]);
-                    dF[0] = fma(8.0, F[1] - Fm1, Fm2 - F[2]);
-                    dH[1] = fma(8.0, H[2] - H[0], Hm1 - H[3]);
-                    dF[1] = fma(8.0, F[2] - F[0], Fm1 - F[3]);
-                    dH[P - 2] = fma(8.0, H[P - 1] - H[P - 3], H[P - 4] - Hp0);
-                    dF[P - 2] = fma(8.0, F[P - 1] - F[P - 3], F[P - 4] - Fp0);
-                    dH[P - 1] = fma(8.0, Hp0 - H[P - 2], H[P - 3] - Hp1);
-                    dF[P - 1] = fma(8.0, Fp0 - F[P - 2], F[P - 3] - Fp1);
                     {
-                        ring_wait(2);
-                        double tC[P];
-#pragma unroll
-                        for (int k = 0; k < 4; ++k) { const double2 m = slot[256 + k * 32 + lane]; tC[2 * k] = m.x; tC[2 * k + 1] = m.y; }
-                        ring_next(2, j);
-#pragma unroll
-                        for (int p = 0; p < P; ++p) {
-                            const double qq = kQ[p];
-                            kP[p] = fma(K.d4c, dH[p], kP[p]);
-                            kQ[p] = fma(tC[p], dF[p], qq);
-                            if (p == 0 && first) {       // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
-                                kP[0] = 0.0;
-                                kQ[0] = fma(8.0 * G1 - G2, K.c_org, qq);
-                            }
+                        const double q0 = kQ[0];
+                        kP[0] = fma(K.d4c, fma(8.0, H[1] - Hm1, Hm2 - H[2]), kP[0]);
+                        kQ[0] = fma(tC[0], fma(8.0, F[1] - Fm1, Fm2 - F[2]), q0);
+                        kP[1] = fma(K.d4c, fma(8.0, H[2] - H[0], Hm1 - H[3]), kP[1]);
+                        kQ[1] = fma(tC[1], fma(8.0, F[2] - F[0], Fm1 - F[3]), kQ[1]);
+                        kP[P - 2] = fma(K.d4c, fma(8.0, H[P - 1] - H[P - 3], H[P - 4] - Hp0), kP[P - 2]);
+                        kQ[P - 2] = fma(tC[P - 2], fma(8.0, F[P - 1] - F[P - 3], F[P - 4] - Fp0), kQ[P - 2]);
+                        kP[P - 1] = fma(K.d4c, fma(8.0, Hp0 - H[P - 2], H[P - 3] - Hp1), kP[P - 1]);
+                        kQ[P - 1] = fma(tC[P - 1], fma(8.0, Fp0 - F[P - 2], F[P - 3] - Fp1), kQ[P - 1]);
+                        if (first) {                     // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
+                            kP[0] = 0.0;
+                            kQ[0] = fma(8.0 * G1 - G2, K.c_org, q0);
                         }
                     }
                     // a5: RK combine; at the first stage u^n is the stage state itself, still in shared memory
@@ -678,10 +685,9 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         }
                         if (last) tot += f7 * (1.0 / 12.0);
                         if (!live) tot = 0.0;
-                        const double incl = warp_suffix_incl(tot);
-                        const double ex = incl - tot;
-                        if (j == 0) ex0 = ex; else if (j == 1) ex1 = ex; else if (j == 2) ex2 = ex; else ex3 = ex;
-                        if (lane == 0) wt[q] = incl;
+#pragma unroll
+                        for (int d = 16; d >= 1; d >>= 1) tot += __shfl_xor_sync(FULL, tot, d);
+                        if (lane == 0) wt[q] = tot;
                     }
                 }   // tiles
             }   // stages
@@ -714,9 +720,10 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     }   // members
 
     // no bulk copy may still be in flight when the CTA's shared memory is released
-    if (pending & 1) ring_wait(0);
-    if (pending & 2) ring_wait(1);
-    if (pending & 4) ring_wait(2);
+    if (n_my > 0) {
+        if (!FIXED) ring_wait(0);
+        ring_wait(1); ring_wait(2);
+    }
 }
 
 // ------------------------------------------------------------------ host side
@@ -769,7 +776,7 @@ cudaError_t launch_stream_async(adsc_ctx *c, long long nsteps, int check_last)
     prm.tabp = c->ws.tabp;
     prm.rec = c->ws.rec; prm.mbox = c->ws.sp_mbox; prm.counter = c->ws.sp_counter;
     prm.nsteps = nsteps; prm.check_last = check_last;
-    prm.G = c->sp_G; prm.groups = c->sp_groups; prm.SQ = c->sp_SQ;
+    prm.G = c->sp_G; prm.groups = c->sp_groups; prm.SQ = c->sp_SQ; prm.zero = 0u;
     {
         const double h = c->pb.h, dt = c->pb.dt, koc = c->pb.ko_eps / (64.0 * h);
         SAConsts &k = prm.k;
