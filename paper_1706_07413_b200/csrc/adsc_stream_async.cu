@@ -45,7 +45,7 @@ constexpr int SA_RS = SA_T + 2;           // 16-byte columns per chunk row of a 
 constexpr int SA_RS3 = SA_T / 2 + 2;      // ... of the fourth (half) tile
 constexpr int SA_TS = 4 * SA_RS;          // tile stride
 constexpr int SA_FS = 3 * SA_TS + 4 * SA_RS3;   // field stride (16-byte units)
-constexpr int SA_MBOX = 24;               // doubles per chunk mailbox
+constexpr int SA_MBOX = 40;               // doubles per chunk mailbox: 17 slots {value, stamp} + padding
 constexpr int SA_SLOT = SA_SL * 8;        // bytes of one table slice
 
 // shared-memory map (bytes)
@@ -83,8 +83,7 @@ struct SAParams {
     double *ACC[3];                  // Runge-Kutta accumulator, permuted
     const double *tabp;              // [NP/256][3][256]: -2 sc, tan^2, cot^2/(12h), permuted for the ring
     MemberRec *rec;
-    double *mbox;                    // [groups][2][G][SA_MBOX]
-    unsigned long long *counter;     // [groups], zeroed before the launch
+    double *mbox;                    // [groups][2][G][SA_MBOX], zeroed before the launch (stamps start at 2)
     long long nsteps;
     int check_last;
     int G, groups, SQ;               // chunks per member, concurrent members, slices per chunk
@@ -97,6 +96,19 @@ __device__ __forceinline__ double ld_cg(const double *p)
     double v;
     asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
     return v;
+}
+
+// One 16-byte mailbox slot {value, stamp}: a single 128-bit transaction each way (STG/LDG.E.128.STRONG.GPU), so a
+// reader that sees the stamp of the round also sees the value that was written with it.
+__device__ __forceinline__ void st_pair(double *p, double v, unsigned long long w)
+{
+    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(__double_as_longlong(v)), "l"(w) : "memory");
+}
+__device__ __forceinline__ void ld_pair(const double *p, double &v, unsigned long long &w)
+{
+    long long a;
+    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(w) : "l"(p) : "memory");
+    v = __longlong_as_double(a);
 }
 
 __host__ __device__ constexpr int sa_rs(int j) { return j < 3 ? SA_RS : SA_RS3; }
@@ -279,9 +291,12 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                 ++stage_ctr;
                 __syncthreads();                                         // S1: state, slice totals, flags of every tile
                 if (warp == 0) {
-                    // ---- a2, slice level: exclusive suffix over the chunk's slices; chunk total and edges to the mailbox
-                    double *mb = prm.mbox + (size_t)gi * 2 * G * SA_MBOX;
-                    double *mine = mb + ((size_t)par * G + c) * SA_MBOX;
+                    // ---- a2, slice level: exclusive suffix over the chunk's slices; the chunk total (with the collapse
+                    // flag in the low bit of its stamp) goes to the chunk's mailbox; then the totals of the chunks above
+                    // are collected as soon as their owners have published them.  Every 16-byte mailbox slot is
+                    // {value, stamp of the round}: one 128-bit store / load each, no fence, no counter, no atomics.
+                    double *mbx = prm.mbox + (size_t)gi * 2 * G * SA_MBOX;
+                    double *mine = mbx + ((size_t)par * G + c) * SA_MBOX;
                     double exq = 0.0;
                     if constexpr (!FIXED) {
                         const double v = (lane < NQ) ? wt[lane] : 0.0;
@@ -289,65 +304,26 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         exq = incl - v;
                         const double fl = (lane < NQ) ? wfl[lane] : 0.0;
                         const int anyf = __any_sync(FULL, fl != 0.0);
-                        if (lane == 0) { mine[0] = incl; mine[1] = anyf ? 1.0 : 0.0; }
-                    }
-                    if (lane < 3) {
-                        mine[2 + lane] = sa_get(S, 0, lane);              mine[5 + lane] = sa_get(S, 1, lane);
-                        mine[10 + lane] = sa_get(S, 0, npts - 3 + lane);  mine[13 + lane] = sa_get(S, 1, npts - 3 + lane);
-                    }
-                    if (!FIXED && lane < 2) { mine[8 + lane] = sa_get(S, 2, lane); mine[16 + lane] = sa_get(S, 2, npts - 2 + lane); }
-                    __threadfence();
-                    __syncwarp();
-                    if (lane == 0) {
-                        unsigned long long *cnt = prm.counter + gi;
-                        const unsigned long long target = (unsigned long long)stage_ctr * (unsigned long long)G;
-                        atomicAdd(cnt, 1ULL);
-                        unsigned long long v;
-                        do {
-                            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(cnt) : "memory");
-                        } while (v < target);
-                    }
-                    __syncwarp();
-                    // ---- gather: totals of the chunks above, flags, neighbour edges / parity ghosts
-                    const double *all = mb + (size_t)par * G * SA_MBOX;
-                    if constexpr (!FIXED) {
-                        double cs = 0.0, fl = 0.0;
+                        if (lane == 0) st_pair(mine, incl, 2ULL * stage_ctr + (anyf ? 1ULL : 0ULL));
+                        const double *all = mbx + (size_t)par * G * SA_MBOX;
+                        double cs = 0.0;
+                        int fls = 0;
                         for (int cc = lane; cc < G; cc += 32) {
-                            const double t = ld_cg(all + (size_t)cc * SA_MBOX), f = ld_cg(all + (size_t)cc * SA_MBOX + 1);
+                            double t;
+                            unsigned long long w;
+                            do { ld_pair(all + (size_t)cc * SA_MBOX, t, w); } while ((w >> 1) != (unsigned long long)stage_ctr);
                             if (cc > c) cs += t;
-                            fl += f;
+                            fls |= (int)(w & 1ULL);
                         }
 #pragma unroll
-                        for (int d = 16; d >= 1; d >>= 1) {
-                            cs += __shfl_xor_sync(FULL, cs, d);
-                            fl += __shfl_xor_sync(FULL, fl, d);
-                        }
+                        for (int d = 16; d >= 1; d >>= 1) cs += __shfl_xor_sync(FULL, cs, d);
+                        fls = __any_sync(FULL, fls);
                         if (lane < NQ) base[lane] = cs + exq;
-                        if (lane == 0) scal[0] = fl;
+                        if (lane == 0) scal[0] = fls ? 1.0 : 0.0;
                     }
-                    if (lane < 3) {
-                        const int k = lane;
-                        if (!phys_lo) {
-                            const double *lo = all + (size_t)(c - 1) * SA_MBOX;
-                            xh[1 + k] = ld_cg(lo + 10 + k); xh[5 + k] = ld_cg(lo + 13 + k);
-                            if (!FIXED && k < 2) xa[k] = ld_cg(lo + 16 + k);
-                        } else {                                         // x = 0: Phi odd, Pi even (R2)
-                            xh[3 - k] = -sa_get(S, 0, 1 + k); xh[7 - k] = sa_get(S, 1, 1 + k);
-                            if (k < 2) xa[k] = 1.0;
-                        }
-                        if (!phys_hi) {
-                            const double *hi = all + (size_t)(c + 1) * SA_MBOX;
-                            xh[8 + k] = ld_cg(hi + 2 + k); xh[12 + k] = ld_cg(hi + 5 + k);
-                            if (!FIXED && k < 2) xa[2 + k] = ld_cg(hi + 8 + k);
-                        } else {                                         // x = pi/2: Phi even, Pi odd, both zero there (R3)
-                            xh[8 + k] = (k == 0) ? 0.0 : sa_get(S, 0, npts - k);
-                            xh[12 + k] = (k == 0) ? 0.0 : -sa_get(S, 1, npts - k);
-                            if (k < 2) xa[2 + k] = 1.0;
-                        }
-                    }
-                    // ---- pre-pass (warp 0): fluxes at the two points below every tile of the chunk and above the chunk,
-                    // which the owner computes later in this stage or in another CTA (one lane per point, full exponential)
-                    __syncwarp();
+                    asm volatile("bar.sync 1, 64;" ::: "memory");        // the chunk halos (warp 1) are in shared memory
+                    // ---- pre-pass: fluxes at the two points below every tile of the chunk and above the chunk, which
+                    // the owner computes later in this stage or in another CTA (one lane per point, full exponential)
                     if (lane < 10) {
                         const int m = lane >> 1, e = lane & 1;
                         const bool top = (m == 4);
@@ -383,13 +359,45 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             dst[2 + e] = etab[6 * m + 4 + e] * Gv;
                         }
                     }
-                } else if (warp == 1 && lane < 24) {
-                    // ---- halo columns at the tile boundaries inside the chunk (the tile below a boundary is full)
-                    const int jb = 1 + (lane >> 3), r = lane & 7, f = r & 1, wh = r >> 1;
-                    if (jb < NT) {
-                        if (wh < 2) S[sa_idx(f, jb, 2 + wh, -1)] = S[sa_idx(f, jb - 1, 2 + wh, SA_T - 1)];
-                        else S[sa_idx(f, jb - 1, wh - 2, SA_T)] = S[sa_idx(f, jb, wh - 2, 0)];
+                } else if (warp == 1) {
+                    // ---- state edges of the chunk to its mailbox; halo columns at the tile boundaries inside the chunk
+                    // (the tile below a boundary is full); the neighbours' edges, or the parity ghosts, to shared memory
+                    double *mbx = prm.mbox + (size_t)gi * 2 * G * SA_MBOX;
+                    double *mine = mbx + ((size_t)par * G + c) * SA_MBOX;
+                    const unsigned long long stamp = 2ULL * stage_ctr;
+                    if (lane < 16 && G > 1) {
+                        // slots 1..8: Phi, Pi at the first three points, A at the first two; 9..16: the same at the last
+                        const int hi = lane >> 3, k = lane & 7;
+                        const int f = (k < 3) ? 0 : (k < 6 ? 1 : 2), off = (k < 3) ? k : (k < 6 ? k - 3 : k - 6);
+                        const int l = hi ? npts - (f == 2 ? 2 : 3) + off : off;
+                        if (!(FIXED && f == 2)) st_pair(mine + 2 * (1 + lane), sa_get(S, f, l), stamp);
                     }
+                    if (lane < 24) {
+                        const int jb = 1 + (lane >> 3), r = lane & 7, f = r & 1, wh = r >> 1;
+                        if (jb < NT) {
+                            if (wh < 2) S[sa_idx(f, jb, 2 + wh, -1)] = S[sa_idx(f, jb - 1, 2 + wh, SA_T - 1)];
+                            else S[sa_idx(f, jb - 1, wh - 2, SA_T)] = S[sa_idx(f, jb, wh - 2, 0)];
+                        }
+                    }
+                    if (lane < 16) {
+                        // lanes 0..7: what lies below the chunk (the LAST points of chunk c-1), 8..15: above (the FIRST of c+1)
+                        const int up = lane >> 3, k = lane & 7;
+                        const int f = (k < 3) ? 0 : (k < 6 ? 1 : 2), off = (k < 3) ? k : (k < 6 ? k - 3 : k - 6);
+                        double v;
+                        if (up ? !phys_hi : !phys_lo) {
+                            const double *src = mbx + ((size_t)par * G + (up ? c + 1 : c - 1)) * SA_MBOX + 2 * (1 + (up ? 0 : 8) + k);
+                            unsigned long long w = 0;
+                            v = 0.0;
+                            if (!(FIXED && f == 2)) { do { ld_pair(src, v, w); } while (w != stamp); }
+                        } else if (!up) {                                // x = 0: Phi odd, Pi even (R2); slot off is point off-3
+                            v = (f == 2) ? 1.0 : (f == 0 ? -sa_get(S, 0, 3 - off) : sa_get(S, 1, 3 - off));
+                        } else {                                         // x = pi/2: Phi even, Pi odd, both zero there (R3)
+                            v = (f == 2) ? 1.0 : (off == 0 ? 0.0 : (f == 0 ? sa_get(S, 0, npts - off) : -sa_get(S, 1, npts - off)));
+                        }
+                        if (f == 2) xa[2 * up + off] = v;
+                        else xh[8 * up + 4 * f + (up ? 0 : 1) + off] = v;
+                    }
+                    asm volatile("bar.sync 1, 64;" ::: "memory");
                 }
                 __syncthreads();                                         // S2
                 if (s == 0) {
@@ -768,13 +776,14 @@ cudaError_t launch_stream_async(adsc_ctx *c, long long nsteps, int check_last)
     const void *fn = c->pb.fixed_bg ? (const void *)k_stream_async<true> : (const void *)k_stream_async<false>;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SA_SMEM);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(c->ws.sp_counter, 0, sizeof(unsigned long long) * SP_MAX_CTAS, c->stream);
+    // mailbox stamps count the barrier rounds of THIS launch from 1: clear what the last launch left behind
+    e = cudaMemsetAsync(c->ws.sp_mbox, 0, sizeof(double) * (size_t)c->sp_groups * 2 * c->sp_G * SA_MBOX, c->stream);
     if (e != cudaSuccess) return e;
     SAParams prm;
     prm.pb = c->pb; prm.tb = c->tb;
     for (int v = 0; v < 3; ++v) { prm.U[v] = c->ws.U[v]; prm.UN[v] = c->ws.Ua[v]; prm.ACC[v] = c->ws.ACC[v]; }
     prm.tabp = c->ws.tabp;
-    prm.rec = c->ws.rec; prm.mbox = c->ws.sp_mbox; prm.counter = c->ws.sp_counter;
+    prm.rec = c->ws.rec; prm.mbox = c->ws.sp_mbox;
     prm.nsteps = nsteps; prm.check_last = check_last;
     prm.G = c->sp_G; prm.groups = c->sp_groups; prm.SQ = c->sp_SQ; prm.zero = 0u;
     {
