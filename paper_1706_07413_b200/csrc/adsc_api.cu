@@ -294,6 +294,7 @@ int adsc_step(adsc_handle h, long long nsteps)
             long long n = left;
             if (K > 0) { const long long to_b = K - (h->global_step % K); if (n > to_b) n = to_b; }
             if (h->steps_per_launch > 0 && n > h->steps_per_launch) n = h->steps_per_launch;
+            if (n > (1LL << 30)) n = 1LL << 30;              // (the kernels count the steps of a launch in 32 bits)
             const bool hit = K > 0 && ((h->global_step + n) % K == 0);
             if (h->path == 2) ADSC_CUDA(launch_resident(h, n, hit ? 0 : 1), "resident kernel");
             else ADSC_CUDA(launch_stream_async(h, n, hit ? 0 : 1), "persistent streaming kernel");

@@ -44,8 +44,9 @@ __device__ __forceinline__ double exp3_ref(double x)
 // e^{x_p} for P values that lie close together: one exp at the reference x_{P-1}, the rest
 // relative to it.  exp(z) = 1 + z t(z), t = sum_{k<=5} z^k/(k+1)!; for |z| <= 2^-6 the truncation
 // is z^7/5040 < 5e-17 relative.  x = 0 gives exactly 1 (pure AdS stays bit-exact).
-template <int P>
-__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P])
+// `scale` multiplies every result (one extra multiplication: it is folded into the reference value).
+template <int P, bool SCALED = false>
+__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], const double scale = 1.0)
 {
     const double xr = x[P - 1];
     double z[P];
@@ -58,7 +59,7 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P])
         mid |= (hz > 0x3f500000) ? 1 : 0;    // |z| > 2^-10
         sml |= (hz > 0x3f100000) ? 1 : 0;    // |z| > 2^-14
     }
-    const double Er = exp3_ref(xr);
+    const double Er = SCALED ? exp3_ref(xr) * scale : exp3_ref(xr);
     E[P - 1] = Er;
     if (!sml) {                              // |z| <= 2^-14: two terms of t suffice (z^4/24 < 6e-19)
 #pragma unroll
@@ -87,7 +88,7 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P])
         }
     } else {
 #pragma unroll
-        for (int p = 0; p < P - 1; ++p) E[p] = exp3_ref(x[p]);
+        for (int p = 0; p < P - 1; ++p) E[p] = SCALED ? exp3_ref(x[p]) * scale : exp3_ref(x[p]);
     }
 }
 

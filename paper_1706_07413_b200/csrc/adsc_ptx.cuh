@@ -77,7 +77,8 @@ __device__ __forceinline__ void bulk_g2s_after_reads(uint32_t dst_smem, const vo
 // 256-bit global accesses (sm_100: LDG.E.256 / STG.E.256), 32-byte aligned.
 __device__ __forceinline__ void ldg256(const double *p, double &a, double &b, double &c, double &d)
 {
-    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
+    // streamed once per use: no L1 allocation (the little L1 left beside 227 KB of shared memory serves the stack)
+    asm volatile("ld.global.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
 }
 __device__ __forceinline__ void stg256(double *p, double a, double b, double c, double d)
 {

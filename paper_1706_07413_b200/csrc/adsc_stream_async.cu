@@ -29,9 +29,6 @@
 #include "adsc_internal.cuh"
 #include "adsc_exp.cuh"
 #include "adsc_ptx.cuh"
-#ifdef SA_DEBUG
-#include <cstdio>
-#endif
 
 namespace adsc {
 
@@ -63,7 +60,7 @@ constexpr int o_xh = o_ftop + 4;          // [16] state halos of the chunk: lowe
 constexpr int o_xa = o_xh + 16;           // [4] A at the two points below / above the chunk
 constexpr int o_esc = o_xa + 4;           // [28][2] -2 sc just below / just above every slice
 constexpr int o_etab = o_esc + 2 * SA_MAXQ;   // [5][6] tables around every boundary the pre-pass serves
-constexpr int o_scal = o_etab + 32;       // [8] scalars: 0 flag sum
+constexpr int o_scal = o_etab + 32;       // [8] scalars: 0 collapse flag of the member, 1 factor C of the chunks above
 constexpr int o_mbar = o_scal + 8;        // mbF, ring[8][3]
 constexpr int SA_MISC_DOUBLES = o_mbar + 26;
 constexpr size_t SA_SMEM = (size_t)SA_OFF_MISC + (size_t)SA_MISC_DOUBLES * 8;
@@ -167,18 +164,19 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     const int NT = (NQ + SA_NW - 1) / SA_NW;             // tiles
     const int n_my = (NQ > warp) ? (NQ - 1 - warp) / SA_NW + 1 : 0;   // this warp owns slices 8 j + warp, j < n_my
     const bool phys_lo = (c == 0), phys_hi = (c == G - 1);
-    const int t_last = npts / P - 1;                     // chunk-level index of the thread that owns the last point
     const int cs0 = c * prm.SQ;                          // first slice of the chunk within a member row
     unsigned stage_ctr = 0;                              // barrier rounds so far; runs on across members, so the
                                                          // mailbox parity never repeats early
 
     const uint32_t mbF = smem_u32(misc + o_mbar);
     const uint32_t mbR = mbF + 8 + (uint32_t)warp * 24;  // this warp's three ring barriers
+    const uint32_t mbC = mbF + 8 * 25;                   // "the factor of the chunks above is in shared memory"
     const uint32_t ringw = smem_u32(smraw + SA_OFF_RING) + (uint32_t)warp * 3 * SA_SLOT;
     const double2 *slot = reinterpret_cast<const double2 *>(smraw + SA_OFF_RING + (size_t)warp * 3 * SA_SLOT);
     if (tid == 0) {
         mbar_init(mbF, SA_NW);
         for (int k = 0; k < 3 * SA_NW; ++k) mbar_init(mbF + 8 + 8 * k, 1);
+        mbar_init(mbC, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // columns of threads that own no point are read as halos by their neighbours: keep them finite
@@ -203,7 +201,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     // ---- table ring: slot t of this warp holds table t (0: -2 sc, 1: tan^2, 2: cot^2/(12h)) of the slice the warp
     // works on next; it is refilled by one bulk copy as soon as the warp has read it.  A warp with a single slice
     // keeps its tables for the whole launch.
-    unsigned rpar = 0;                                   // phase parity per slot
+    unsigned phs = 0;                                    // phase parities: bits 0..2 ring slots, 3 mbF, 4 mbC
     const bool reload = n_my > 1;
     auto ring_issue = [&](int t, int qn, unsigned dep) {
         if (lane == 0) {
@@ -216,7 +214,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
         if (!FIXED) ring_issue(0, q0, 0u);
         ring_issue(1, q0, 0u); ring_issue(2, q0, 0u);
     }
-    auto ring_wait = [&](int t) { mbar_wait<false>(mbR + 8 * t, (rpar >> t) & 1u); };
+    auto ring_wait = [&](int t) { mbar_wait<false>(mbR + 8 * t, (phs >> t) & 1u); };
     // After the warp has read slot t of slice q (tile j): fetch the same table of its next slice.  The copy engine is
     // not ordered behind the warp's shared-memory loads, so the copy is made to DEPEND on them: `dep` mixes one word of
     // every load of the slot into the byte count (and with a run-time zero), and the copy is predicated on the state
@@ -225,14 +223,36 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
         if (reload) {
             dep = __reduce_or_sync(FULL, dep);
             ring_issue(t, SA_NW * (j > 0 ? j - 1 : n_my - 1) + warp, dep);
-            rpar ^= 1u << t;
+            phs ^= 1u << t;
         }
     };
 
-    unsigned ftick = 0;                                  // tile iterations since the kernel started (phase of mbF)
     auto warp_arrive = [&](uint32_t mbx) {
         __syncwarp();
         if (lane == 0) mbar_arrive(mbx);
+    };
+    // a2, chunk level.  The chunks above this one enter delta only through ONE number, the sum cs of their totals of
+    // f', and e^{-delta} = C e^{-delta_local} with C = e^{(h/2) cs}: every flux of the chunk is linear in C.  So a stage
+    // does not wait for the other CTAs before it starts: it works with delta_local, and one warp collects the totals
+    // (stamped mailbox slots, see st_pair) when the first tile of the stage is about to need C -- by then the
+    // other CTAs have long published theirs.  The warp leaves the collapse flag of the member and C in shared
+    // memory and arrives on mbC.  e^0 = 1 exactly: pure AdS stays bit-exact.
+    auto gather = [&](const int par) {
+        const double *all = prm.mbox + ((size_t)gi * 2 + par) * G * SA_MBOX;
+        double cs = 0.0;
+        int fls = 0;
+        for (int cc = lane; cc < G; cc += 32) {
+            double t;
+            unsigned long long w;
+            do { ld_pair(all + (size_t)cc * SA_MBOX, t, w); } while ((w >> 1) != (unsigned long long)stage_ctr);
+            if (cc > c) cs += t;
+            fls |= (int)(w & 1ULL);
+        }
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) cs += __shfl_xor_sync(FULL, cs, d);
+        fls = __any_sync(FULL, fls);
+        if (lane == 0) { scal[0] = fls ? 1.0 : 0.0; scal[1] = exp3_ref(K.hh * cs); }
+        warp_arrive(mbC);
     };
 
     for (int b = gi; b < pb.B; b += prm.groups) {
@@ -277,13 +297,13 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     tot += fa + fb;
                     if (k == 3) f7 = fb;
                 }
-                if (phys_hi && (l0 >> 3) == t_last) tot += f7 * (1.0 / 12.0);    // top term of the telescoped rule
+                if (phys_hi && l0 + P == npts) tot += f7 * (1.0 / 12.0);    // top term of the telescoped rule
                 const double incl = warp_suffix_incl(tot);
                 if (lane == 0) { wt[q] = incl; wfl[q] = 0.0; }
             }
         }
         int collapsed = 0;
-        long long n = 0;
+        int n = 0;                                                   // (the host splits calls of more than 2^30 steps)
 
         for (;;) {
             for (int s = 0; s < NS; ++s) {
@@ -292,8 +312,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                 __syncthreads();                                         // S1: state, slice totals, flags of every tile
                 if (warp == 0) {
                     // ---- a2, slice level: exclusive suffix over the chunk's slices; the chunk total (with the collapse
-                    // flag in the low bit of its stamp) goes to the chunk's mailbox; then the totals of the chunks above
-                    // are collected as soon as their owners have published them.  Every 16-byte mailbox slot is
+                    // flag in the low bit of its stamp) goes to the chunk's mailbox.  Every 16-byte mailbox slot is
                     // {value, stamp of the round}: one 128-bit store / load each, no fence, no counter, no atomics.
                     double *mbx = prm.mbox + (size_t)gi * 2 * G * SA_MBOX;
                     double *mine = mbx + ((size_t)par * G + c) * SA_MBOX;
@@ -305,21 +324,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         const double fl = (lane < NQ) ? wfl[lane] : 0.0;
                         const int anyf = __any_sync(FULL, fl != 0.0);
                         if (lane == 0) st_pair(mine, incl, 2ULL * stage_ctr + (anyf ? 1ULL : 0ULL));
-                        const double *all = mbx + (size_t)par * G * SA_MBOX;
-                        double cs = 0.0;
-                        int fls = 0;
-                        for (int cc = lane; cc < G; cc += 32) {
-                            double t;
-                            unsigned long long w;
-                            do { ld_pair(all + (size_t)cc * SA_MBOX, t, w); } while ((w >> 1) != (unsigned long long)stage_ctr);
-                            if (cc > c) cs += t;
-                            fls |= (int)(w & 1ULL);
-                        }
-#pragma unroll
-                        for (int d = 16; d >= 1; d >>= 1) cs += __shfl_xor_sync(FULL, cs, d);
-                        fls = __any_sync(FULL, fls);
-                        if (lane < NQ) base[lane] = cs + exq;
-                        if (lane == 0) scal[0] = fls ? 1.0 : 0.0;
+                        if (lane < NQ) base[lane] = exq;                   // within the chunk (see `gather`)
                     }
                     asm volatile("bar.sync 1, 64;" ::: "memory");        // the chunk halos (warp 1) are in shared memory
                     // ---- pre-pass: fluxes at the two points below every tile of the chunk and above the chunk, which
@@ -400,19 +405,34 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     asm volatile("bar.sync 1, 64;" ::: "memory");
                 }
                 __syncthreads();                                         // S2
-                if (s == 0) {
-                    // a6: collapse test of PAPER.md:85 on the state after n steps (flags of every chunk)
-                    if (!FIXED && n > 0 && scal[0] != 0.0) { collapsed = 1; break; }
-                    if (n == prm.nsteps) break;                          // final flag round only
+                if (s == 0 && n == prm.nsteps) {                         // final flag round only: nothing to overlap
+                    if constexpr (!FIXED) {
+                        const uint32_t cpar = (phs >> 4) & 1u;
+                        phs ^= 16u;
+                        if (warp == SA_NW - 1) gather(par);
+                        mbar_wait<false>(mbC, cpar);
+                        // a6: collapse test of PAPER.md:85 on the state after n steps (flags of every chunk)
+                        if (n > 0 && scal[0] != 0.0) collapsed = 1;
+                    }
+                    break;
                 }
-                // dead lanes (points beyond i = N-2 in the top chunk) keep their (zero) state: weights 0
-                const double a_n = K.a_next[s], b_n = K.b_w[s];
 
                 // ---- tiles
+                double Cst = 1.0;                                         // C, once this stage's gather is done
+                const uint32_t cpar = (phs >> 4) & 1u;
+                phs ^= 16u;
                 for (int j = NT - 1; j >= 0; --j) {
-                    const uint32_t fpar = ftick & 1u;
-                    ++ftick;
+                    // the first tile of the stage works with delta_local and takes C in at its end
+                    const bool defer = !FIXED && (j == NT - 1);
                     if (j >= n_my) {                                      // ragged top tile: nothing to do for this warp
+                        if (defer) {
+                            if (warp == SA_NW - 1) gather(par);
+                            mbar_wait<false>(mbC, cpar);
+                            Cst = scal[1];
+                            if (s == 0 && n > 0 && scal[0] != 0.0) { collapsed = 1; break; }     // a6
+                        }
+                        const uint32_t fpar = (phs >> 3) & 1u;
+                        phs ^= 8u;
                         warp_arrive(mbF);
                         mbar_wait<false>(mbF, fpar);
                         continue;
@@ -422,9 +442,10 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     const int tch = l0 >> 3;                              // chunk-level thread index
                     const bool live = l0 < npts;
                     const bool first = phys_lo && tch == 0;               // owns i = 0
-                    const bool last = phys_hi && tch == t_last;           // owns i = N-2; i = N-1 is its halo
+                    const bool last = phys_hi && l0 + P == npts;          // owns i = N-2; i = N-1 is its halo
                     const int R = sa_rs(j);
-                    const double a_next = live ? a_n : 0.0, b_w = live ? b_n : 0.0;
+                    // dead lanes (points beyond i = N-2 in the top chunk) keep their (zero) state: weights 0
+                    const double a_next = live ? K.a_next[s] : 0.0, b_w = live ? K.b_w[s] : 0.0;
                     double2 *sP = S + sa_idx(0, j, 0, tid);
                     // permuted u^n / accumulator of this thread's points
                     const size_t po = prow + (size_t)q * SA_SL + lane * 4;
@@ -441,7 +462,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         const double2 *l2 = sP - 1 + 2 * R, *l3 = sP - 1 + 3 * R, *h0 = sP + 1, *h1 = sP + 1 + R;
                         int fol = SA_FS, foh = SA_FS;
                         if (tch == 0) { l2 = xh2; l3 = xh2 + 1; fol = 2; }
-                        if (tch == t_last) { h0 = xh2 + 4; h1 = xh2 + 5; foh = 2; }
+                        if (l0 + P == npts) { h0 = xh2 + 4; h1 = xh2 + 5; foh = 2; }
                         const double2 u2 = l2[0], u3 = l3[0], w2 = l2[fol], w3 = l3[fol];
                         hlP[0] = u2.y; hlP[1] = u3.x; hlP[2] = u3.y; hlQ[0] = w2.y; hlQ[1] = w3.x; hlQ[2] = w3.y;
                         const double2 v0 = h0[0], v1 = h1[0], y0 = h0[foh], y1 = h1[foh];
@@ -504,10 +525,8 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             loc = fma(-K.c1, f_lo, loc);
                             nd[p] = fma(K.hh, s2 + B, loc);
                         }
-                        exp3_near<P>(nd, E);
-#ifdef SA_DEBUG
-                        if (blockIdx.x == 0 && warp == 0 && lane < 4 && n == 0) printf("s%d lane%d B=%g base=%g so0=%g fm=%g fp=%g nd0=%g nd7=%g E0=%g E7=%g ph0=%g ph7=%g m2_0=%g m2_7=%g hlP=%g %g %g hrP=%g %g %g\n", s, lane, B, base[q], so[0], fm, fp, nd[0], nd[7], E[0], E[7], ph[0], ph[7], m2[0], m2[7], hlP[0], hlP[1], hlP[2], hrP[0], hrP[1], hrP[2]);
-#endif
+                        if (defer) exp3_near<P>(nd, E);
+                        else exp3_near<P, true>(nd, E, Cst);
                     }
                     // global operands of the A update (needed at the end of phase 1)
                     double unA[P], acA[P];
@@ -522,7 +541,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         }
                     }
                     // a3 fluxes
-                    double H[P], F[P], kAv[P], a[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
+                    double H[P], F[P], kAv[P], a[P], Gorg = 0.0, Gtop = 0.0;   // 8 G_1 - G_2 (R4) and 16 G_{P-1} - G_{P-2} (R5)
                     {
                         ring_wait(1);
                         double tT[P];
@@ -544,15 +563,31 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             const double Gv = AE * ph[p];
                             H[p] = AE * pi[p];
                             F[p] = tT[p] * Gv;
-                            if (p == 1) G1 = Gv;
-                            if (p == 2) G2 = Gv;
-                            if (p == P - 1) Gl1 = Gv;
-                            if (p == P - 2) Gl2 = Gv;
+                            if (p == 1) Gorg = 8.0 * Gv;
+                            if (p == 2) Gorg -= Gv;
+                            if (p == P - 2) Gtop = -Gv;
+                            if (p == P - 1) Gtop = fma(16.0, Gv, Gtop);
                             if constexpr (FIXED) kAv[p] = 0.0;                    // A = 1 held fixed
                             else kAv[p] = (m2[p] * a[p]) * (Gv * pi[p]);          // eq (4): -2 sc A G Pi
                         }
                     }
                     if (first) kAv[0] = 0.0;                                      // A(0,t)=1, eq (8)
+                    if (defer) {
+                        if (warp == SA_NW - 1) gather(par);
+                        mbar_wait<false>(mbC, cpar);
+                        Cst = scal[1];
+                        if (s == 0 && n > 0 && scal[0] != 0.0) {                  // a6: nothing has been changed yet
+                            if (reload) {                                         // the ring is ahead by one slice: put it back
+                                const int q0 = SA_NW * (n_my - 1) + warp;
+                                ring_wait(0); ring_issue(0, q0, 0u); phs ^= 1u;
+                                ring_wait(1); ring_issue(1, q0, 0u); phs ^= 2u;
+                            }
+                            collapsed = 1;
+                            break;
+                        }
+                    }
+                    const double Cl = defer ? Cst : 1.0;                          // what is still to be multiplied in
+                    const double a_nC = a_next * Cl, b_wC = b_w * Cl;
                     // a4/a5 for A (eq 4 needs no neighbour)
                     if constexpr (!FIXED) {
                         double aN[P];
@@ -560,8 +595,8 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             double accn[P];
 #pragma unroll
                             for (int p = 0; p < P; ++p) {
-                                accn[p] = fma(b_w, kAv[p], (s == 0) ? a[p] : acA[p]);
-                                aN[p] = fma(a_next, kAv[p], (s == 0) ? a[p] : unA[p]);
+                                accn[p] = fma(b_wC, kAv[p], (s == 0) ? a[p] : acA[p]);
+                                aN[p] = fma(a_nC, kAv[p], (s == 0) ? a[p] : unA[p]);
                             }
                             stg256(prm.ACC[2] + po, accn[0], accn[1], accn[2], accn[3]);
                             stg256(prm.ACC[2] + po + 128, accn[4], accn[5], accn[6], accn[7]);
@@ -570,7 +605,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             int bad = 0;
 #pragma unroll
                             for (int p = 0; p < P; ++p) {
-                                aN[p] = fma(b_w, kAv[p], acA[p]);
+                                aN[p] = fma(b_wC, kAv[p], acA[p]);
                                 if (!(aN[p] >= K.thr)) bad = 1;                   // a6
                             }
                             stg256(prm.UN[2] + po, aN[0], aN[1], aN[2], aN[3]);
@@ -595,13 +630,11 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             ldg256(prm.UN[1] + po + 128, unQ[4], unQ[5], unQ[6], unQ[7]);
                         }
                     }
-                    // flux edges: neighbour lanes by shuffle, neighbour warps through shared memory
-                    double Hm2 = __shfl_up_sync(FULL, H[P - 2], 1), Hm1 = __shfl_up_sync(FULL, H[P - 1], 1);
-                    double Fm2 = __shfl_up_sync(FULL, F[P - 2], 1), Fm1 = __shfl_up_sync(FULL, F[P - 1], 1);
-                    double Hp0 = __shfl_down_sync(FULL, H[0], 1), Hp1 = __shfl_down_sync(FULL, H[1], 1);
-                    double Fp0 = __shfl_down_sync(FULL, F[0], 1), Fp1 = __shfl_down_sync(FULL, F[1], 1);
+                    // flux edges for the neighbour warps through shared memory (neighbour lanes: shuffles, after the wait)
                     if (lane == 0) { flo2[2 * q] = make_double2(H[0], H[1]); flo2[2 * q + 1] = make_double2(F[0], F[1]); }
                     if (lane == 31) { fhi2[2 * q] = make_double2(H[P - 2], H[P - 1]); fhi2[2 * q + 1] = make_double2(F[P - 2], F[P - 1]); }
+                    const uint32_t fpar = (phs >> 3) & 1u;
+                    phs ^= 8u;
                     warp_arrive(mbF);                                             // sync F: arrive
 
                     // ------------------------------------------------------------ between arrive and wait
@@ -612,42 +645,54 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const double2 m = slot[256 + k * 32 + lane]; tC[2 * k] = m.x; tC[2 * k + 1] = m.y; }
                     ring_next(2, j, (unsigned)(__double2hiint(tC[0]) | __double2hiint(tC[2]) | __double2hiint(tC[4]) | __double2hiint(tC[6])));
+                    const double d4cC = K.d4c * Cl;
+                    if (defer) {
+#pragma unroll
+                        for (int p = 0; p < P; ++p) tC[p] *= Cl;
+                    }
 #pragma unroll
                     for (int p = 2; p < P - 2; ++p) {
-                        kP[p] = fma(K.d4c, fma(8.0, H[p + 1] - H[p - 1], H[p - 2] - H[p + 2]), kP[p]);
+                        kP[p] = fma(d4cC, fma(8.0, H[p + 1] - H[p - 1], H[p - 2] - H[p + 2]), kP[p]);
                         kQ[p] = fma(tC[p], fma(8.0, F[p + 1] - F[p - 1], F[p - 2] - F[p + 2]), kQ[p]);
                     }
                     mbar_wait<false>(mbF, fpar);                                  // sync F: wait
 
                     // ------------------------------------------------------------ phase 2
+                    double Hm2 = __shfl_up_sync(FULL, H[P - 2], 1), Hm1 = __shfl_up_sync(FULL, H[P - 1], 1);
+                    double Fm2 = __shfl_up_sync(FULL, F[P - 2], 1), Fm1 = __shfl_up_sync(FULL, F[P - 1], 1);
+                    double Hp0 = __shfl_down_sync(FULL, H[0], 1), Hp1 = __shfl_down_sync(FULL, H[1], 1);
+                    double Fp0 = __shfl_down_sync(FULL, F[0], 1), Fp1 = __shfl_down_sync(FULL, F[1], 1);
+                    // (the pre-pass and the first tile of the stage leave fluxes WITHOUT the factor C)
                     if (lane == 0) {
                         const double2 *src = (warp == 0) ? fpre2 + 2 * j : fhi2 + 2 * (q - 1);
                         const double2 x = src[0], y = src[1];
-                        Hm2 = x.x; Hm1 = x.y; Fm2 = y.x; Fm1 = y.y;
+                        const double m = (warp == 0 && !defer) ? Cst : 1.0;
+                        Hm2 = x.x * m; Hm1 = x.y * m; Fm2 = y.x * m; Fm1 = y.y * m;
                     }
                     if (lane == 31) {
                         const double2 *src = (q + 1 < NQ) ? flo2 + 2 * (q + 1) : ftop2;
                         const double2 x = src[0], y = src[1];
-                        Hp0 = x.x; Hp1 = x.y; Fp0 = y.x; Fp1 = y.y;
+                        const double m = (!FIXED && !defer && q + 1 == SA_NW * (NT - 1)) ? Cst : 1.0;
+                        Hp0 = x.x * m; Hp1 = x.y * m; Fp0 = y.x * m; Fp1 = y.y * m;
                     }
                     if (first) { Hm2 = H[2]; Hm1 = H[1]; Fm2 = -F[2]; Fm1 = -F[1]; }      // x=0: H even, F odd
                     if (last) {                                                   // x=pi/2: H odd with H=0 there; F even, limit of R5
                         Hp0 = 0.0; Hp1 = -H[P - 1];
-                        Fp0 = (16.0 * Gl1 - Gl2) * K.inv12h2; Fp1 = F[P - 1];
+                        Fp0 = Gtop * K.inv12h2; Fp1 = F[P - 1];
                     }
                     {
                         const double q0 = kQ[0];
-                        kP[0] = fma(K.d4c, fma(8.0, H[1] - Hm1, Hm2 - H[2]), kP[0]);
+                        kP[0] = fma(d4cC, fma(8.0, H[1] - Hm1, Hm2 - H[2]), kP[0]);
                         kQ[0] = fma(tC[0], fma(8.0, F[1] - Fm1, Fm2 - F[2]), q0);
-                        kP[1] = fma(K.d4c, fma(8.0, H[2] - H[0], Hm1 - H[3]), kP[1]);
+                        kP[1] = fma(d4cC, fma(8.0, H[2] - H[0], Hm1 - H[3]), kP[1]);
                         kQ[1] = fma(tC[1], fma(8.0, F[2] - F[0], Fm1 - F[3]), kQ[1]);
-                        kP[P - 2] = fma(K.d4c, fma(8.0, H[P - 1] - H[P - 3], H[P - 4] - Hp0), kP[P - 2]);
+                        kP[P - 2] = fma(d4cC, fma(8.0, H[P - 1] - H[P - 3], H[P - 4] - Hp0), kP[P - 2]);
                         kQ[P - 2] = fma(tC[P - 2], fma(8.0, F[P - 1] - F[P - 3], F[P - 4] - Fp0), kQ[P - 2]);
-                        kP[P - 1] = fma(K.d4c, fma(8.0, Hp0 - H[P - 2], H[P - 3] - Hp1), kP[P - 1]);
+                        kP[P - 1] = fma(d4cC, fma(8.0, Hp0 - H[P - 2], H[P - 3] - Hp1), kP[P - 1]);
                         kQ[P - 1] = fma(tC[P - 1], fma(8.0, Fp0 - F[P - 2], F[P - 3] - Fp1), kQ[P - 1]);
                         if (first) {                     // Phi(0,t)=0 (eq 7); Pi_dot(0) = 3 (A e^{-delta} Phi)'(0) (R4)
                             kP[0] = 0.0;
-                            kQ[0] = fma(8.0 * G1 - G2, K.c_org, q0);
+                            kQ[0] = fma(Gorg, K.c_org * Cl, q0);
                         }
                     }
                     // a5: RK combine; at the first stage u^n is the stage state itself, still in shared memory
@@ -698,6 +743,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         if (lane == 0) wt[q] = tot;
                     }
                 }   // tiles
+                if (collapsed) break;
             }   // stages
             if (collapsed || n == prm.nsteps) break;
             ++n;
@@ -720,7 +766,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
             }
         }
         if (c == 0 && tid == 0) {
-            const long long sd = rec->steps_done + n;
+            const long long sd = rec->steps_done + (long long)n;
             rec->steps_done = sd;
             if (collapsed) { rec->collapsed = 1; rec->t_collapse = (double)sd * pb.dt; }
         }
