@@ -3,8 +3,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl reference]
 
-One bench "step" = `--rk4-per-step` (default 100) classical RK4 steps of the whole ensemble
-through ONE adsc_step call: every row of SURVEY.md 8(a) (a1-a6) runs 4x per RK4 step.
+One bench "step" = `--rk4-per-step` (default: RK4_PER_STEP below, 1200 for cfg2) classical RK4 steps of the whole
+ensemble through ONE adsc_step call: every row of SURVEY.md 8(a) (a1-a6) runs 4x per RK4 step.  The defaults
+give >= 2 s of timed GPU work with --steps 20 (SURVEY.md 8(d) protocol).
 The N=1 workload is BASELINE.json configs[1] (1024 members, N=4097).  Prints ONE JSON line.
 See DESIGN.md "Measurement" for the definitions used here.
 """
@@ -39,43 +40,53 @@ BYTES_PER_POINT_STEP = 384.0
 # measured DFMA issue rate on this pool is recorded there too).
 FP64_LANES_PER_SM = 64
 N_SMS = 148
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE stage-kernel launch from the committed `ncu --set full`
-# captures (profiles/r01_summary.md).  The state is loaded and stored once per launch whatever the number of
-# RK4 steps in it (resident path) or stays L2-resident (cfg4), so the figure does not scale with rk4_per_step.
-NCU_TRAFFIC_BYTES = {"cfg2": 148.4e6, "cfg5": 1562.0e6, "cfg3": 1563.0e6, "cfg4": 339.1e6, "cfg1": None}
+# Global-memory bytes per point per RK stage the persistent streaming kernel provably moves (u^n and accumulator
+# in the permuted arrays; the stage state never leaves shared memory): classical RK4 = 24 (stage 1: accumulator
+# written) + 72 + 72 (u^n read, accumulator read and written) + 48 (accumulator read, u^n written) = 216 B per
+# point per step, plus 3 coefficient tables x 8 B per stage staged by bulk copies.
+STREAM_BYTES_STAGE_FIRST, STREAM_BYTES_STAGE_MID, STREAM_BYTES_STAGE_LAST, STREAM_BYTES_TABLES = 24.0, 72.0, 48.0, 24.0
+L2_BYTES = 126e6
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="adsc", choices=["adsc", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "paper32k"])
     ap.add_argument("--rk4-per-step", type=int, default=0, help="RK4 steps per bench step (0 = workload default)")
     ap.add_argument("--batch", type=int, default=0, help="override the ensemble size (0 = workload default)")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 persistent streaming, 2 resident, 3 generic streaming")
     ap.add_argument("--fixed-background", action="store_true",
                     help="time the fixed-background variant (A = 1, delta = 0 held fixed; PAPER.md:177 Table II)")
-    ap.add_argument("--rk-order", type=int, default=4, choices=[2, 3, 4],
+    ap.add_argument("--rk-order", type=int, default=0, choices=[0, 2, 3, 4],
                     help="Runge-Kutta order (PAPER.md:57; 3 and 2 run on the streaming paths); the metric then counts "
-                         "grid-point steps of that rule and the algorithmic cost scales with the stage count")
+                         "grid-point steps of that rule and the algorithmic cost scales with the stage count "
+                         "(0 = workload default: 4, except paper32k: 3)")
     ap.add_argument("--masked-fraction", type=float, default=0.0,
                     help="force this fraction of the members to collapse during warm-up (Pi x 1000): shows that masked "
                          "members cost nothing; the metric then counts the members still active (SURVEY.md 8(d))")
     ap.add_argument("--e2e-parts", type=int, default=8, help="sub-batches (handles, streams) of the e2e leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
-    return ap.parse_args()
+    ap.add_argument("--probe-ms", type=float, default=50.0, help="duration of each roofline-denominator probe (0 = skip)")
+    a = ap.parse_args()
+    if a.rk_order == 0:
+        a.rk_order = 3 if a.workload == "paper32k" else 4
+    return a
 
 
-RK4_PER_STEP = {"cfg1": 2000, "cfg2": 100, "cfg3": 50, "cfg4": 20, "cfg5": 100}
+# RK steps per bench step: >= 100 ms per adsc_step call, so that --steps 20 times >= 2 s of GPU work
+RK4_PER_STEP = {"cfg1": 20000, "cfg2": 1200, "cfg3": 150, "cfg4": 1500, "cfg5": 200, "paper32k": 1000}
 WORKLOAD_DESC = {
     "cfg1": "configs[0]: 1 member, N=1025, Gaussian Pi sigma=1/16 eps=1",
     "cfg2": "configs[1]: amplitude ensemble, 1024 members, N=4097, Gaussian Pi sigma=1/16 eps~U[0.5,5]",
     "cfg3": "configs[2]: two-mode ensemble, 4096 members, N=8193",
     "cfg4": "configs[3]: single large grid, 1 member, N=2^20+1",
     "cfg5": "configs[4]: wide-pulse ensemble, 16384 members, N=2049",
+    "paper32k": "the paper's production shape (PAPER.md:57, 115, 123): 64 amplitudes of the k_d=3, mu=1 family of "
+                "eq (13), N=2^15+1, RK3",
 }
 
 
@@ -130,15 +141,16 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False, rk_order=4):
+def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False, rk_order=4, threads=None):
     """Time the oracle as it stands on the host cores on a bounded sample of the workload:
-    2 x cores members (or the whole batch if smaller), enough RK4 steps for ~`seconds`."""
+    2 x cores members (or the whole batch if smaller), enough RK4 steps for ~`seconds`.
+    threads=1: the one-core, one-member leg of SURVEY.md 8(d)(i)."""
     import oracle
     from paper_1706_07413_b200 import inputs
     cores = os.cpu_count() or 1
-    thr = min(cores, oracle.max_threads())
+    thr = min(cores, oracle.max_threads()) if threads is None else threads
     Bfull = inputs.CONFIGS[name]["B"]
-    B = min(Bfull, 2 * thr)
+    B = min(Bfull, 2 * thr) if threads is None else threads
     thr = min(thr, B)
     Phi, Pi, _ = inputs.make(name, B=B)
     ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=fixed, rk_order=rk_order)
@@ -228,13 +240,13 @@ def main():
 
     # Rank r evolves members [r*B, (r+1)*B) of the (tiled) seeded ensemble: no exchange step.
     lo, hi = shard.member_range(rank, world, B * world)
-    Phi_all, Pi_all, _ = inputs.make(name, B=hi)
+    Phi_all, Pi_all, _ = inputs.make(name, B=hi, lo=lo)       # this rank's members only
     if args.masked_fraction > 0.0:
         bidx = np.arange(lo, hi)
         forced = np.floor((bidx + 1) * args.masked_fraction) > np.floor(bidx * args.masked_fraction)
-        Pi_all[lo:hi][forced] *= 1.0e3            # collapses within the first warm-up steps
-    Phi_h = torch.from_numpy(np.ascontiguousarray(Phi_all[lo:hi])).pin_memory()
-    Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all[lo:hi])).pin_memory()
+        Pi_all[forced] *= 1.0e3                   # collapses within the first warm-up steps
+    Phi_h = torch.from_numpy(np.ascontiguousarray(Phi_all)).pin_memory()
+    Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all)).pin_memory()
     del Phi_all, Pi_all
 
     ens = binding.Ensemble(N, B, device=dev, path=args.path, 
@@ -248,6 +260,12 @@ def main():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize(dev)
+
+    # ---- roofline denominators measured on this device, before the timed region (adsc_probe)
+    probe = None
+    if args.probe_ms > 0.0 and rank == 0:
+        probe = {"fp64_fma_tflops": binding.adsc_probe(binding.ADSC_PROBE_FP64_FMA, args.probe_ms) / 1e12,
+                 "shared_load_tbs": binding.adsc_probe(binding.ADSC_PROBE_SHARED_LOAD, args.probe_ms) / 1e12}
 
     # ---- device-resident timing: K bench steps, each one adsc_step(rk4) call
     for _ in range(W):
@@ -319,37 +337,61 @@ def main():
 
     peaks = load_peaks()
     per_gpu_rate = value / world
+    NS = args.rk_order
+    peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
+    slots = (SLOTS_PER_POINT_STEP_FIXED if args.fixed_background else SLOTS_PER_POINT_STEP) * NS / 4.0
+    ach_tf = per_gpu_rate * slots * 2 / 1e12
+    peak_src = (f"derived: {N_SMS} SMs x {FP64_LANES_PER_SM} DFMA lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 flop "
+                f"(DESIGN.md Roofline); peak_measured: adsc_probe(FP64_FMA) run for {args.probe_ms:.0f} ms before "
+                f"the timed region")
+    fp64_meas = probe["fp64_fma_tflops"] if probe else None
     if path == 2:
-        peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
-        slots = (SLOTS_PER_POINT_STEP_FIXED if args.fixed_background else SLOTS_PER_POINT_STEP) * args.rk_order / 4.0
-        ach_tf = per_gpu_rate * slots * 2 / 1e12
         roof = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(name) if (B == cfg["B"] and not args.fixed_background) else None,
-                "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
-                "kernel": "k_resident3 (whole RK4 steps on chip; 1 launch per adsc_step)",
-                "peak_src": f"derived: {N_SMS} SMs x {FP64_LANES_PER_SM} DFMA lanes x "
-                            f"{peaks['sm_max_mhz']:.0f} MHz x 2 flop (DESIGN.md Roofline)",
-                "algorithmic": f"{slots:.0f} FP64-pipe instr per point per RK4 step"}
+                "frac": ach_tf / peak_tf,
+                "peak_measured": fp64_meas, "frac_of_measured": (ach_tf / fp64_meas) if fp64_meas else None,
+                "shared_load_tbs_measured": probe["shared_load_tbs"] if probe else None,
+                "traffic": 6.0 * B * N * 8,
+                "traffic_unit": "global-memory bytes per launch: the three fields are loaded once and stored once, whatever "
+                                "the number of steps in the launch (the ncu dram figures are in profiles/)",
+                "kernel": f"k_resident3 (whole RK steps on chip; {launches // max(K, 1)} launch per adsc_step)",
+                "peak_src": peak_src,
+                "algorithmic": f"{slots:.0f} FP64-pipe instr per point per step"}
     else:
-        # streaming bytes per step: first and last stage 72 B, every middle stage 120 B
-        bytes_step = 72.0 * 2 + 120.0 * (args.rk_order - 2)
+        # [NS]/SURVEY.md 8(d) streaming roofline: bytes per point per step with one fused pass per stage:
+        # first and last stage 72 B, every middle stage 120 B
+        bytes_step = 72.0 * 2 + 120.0 * (NS - 2)
         ach = per_gpu_rate * bytes_step / 1e9
+        kern_bytes = (STREAM_BYTES_STAGE_FIRST + STREAM_BYTES_STAGE_LAST + STREAM_BYTES_STAGE_MID * (NS - 2)
+                      + STREAM_BYTES_TABLES * NS)
+        wset = 9.0 * B * N * 8 + 3.0 * N * 8
         roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(name) if (B == cfg["B"] and not args.fixed_background) else None,
-                "traffic_unit": "bytes per launch (ncu, profiles/r01_summary.md)",
-                "kernel": ("k_stream_persist (stage state in shared memory, u^n/accumulator through L2; "
-                           "1 cooperative launch per adsc_step)" if path == 1 else
+                "frac": ach / peaks["hbm_gbs"],
+                "traffic": (kern_bytes * rk4 + 48.0) * B * N if path == 1 else None,
+                "traffic_unit": "global-memory bytes per launch the kernel provably requests (u^n, accumulator, tables; "
+                                "load + store of the fields once); see l2_resident",
+                "kernel_bytes_per_point_step": kern_bytes if path == 1 else None,
+                "working_set_bytes": wset, "l2_resident": bool(wset < L2_BYTES),
+                "alu": {"achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
+                        "peak_measured": fp64_meas, "frac_of_measured": (ach_tf / fp64_meas) if fp64_meas else None},
+                "note": ("the [NS] streaming roofline (algorithmic bytes over the HBM copy peak); when l2_resident is true "
+                         "the working set never leaves the 126 MB L2, HBM is not the binding resource and the `alu` "
+                         "fraction is the one that measures the kernel"),
+                "kernel": ("k_stream_async (stage state in shared memory, tables staged by cp.async.bulk rings, "
+                           "u^n/accumulator through L2; 1 cooperative launch per adsc_step)" if path == 1 else
                            "k_stream_rhs (+ k_stream_I, k_stream_carry: 3 launches per RK stage)"),
-                "peak_src": f"{peaks['src']} copy bandwidth (MEASURED_PEAKS.json)",
+                "peak_src": f"{peaks['src']} copy bandwidth (MEASURED_PEAKS.json); alu: " + peak_src,
                 "algorithmic": f"{bytes_step:.0f} B per point per step"}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         cpu, _, _, _ = oracle_rate(name, N, args.cpu_seconds, fixed=args.fixed_background, rk_order=args.rk_order)
+        one, _, _, _ = oracle_rate(name, N, min(5.0, args.cpu_seconds), fixed=args.fixed_background,
+                                   rk_order=args.rk_order, threads=1)
+        cpu["one_core"] = {"value": one["value"], "unit": UNIT, "cores": 1, "sample": one["sample"]}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / K, "timed_region_s": ms * 1e-3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic (seeded, paper_1706_07413_b200/inputs.py)",
         "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_per_gpu": B, "global_batch": B * world,
                    "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1, "fixed_background": bool(args.fixed_background), "rk_order": args.rk_order,

@@ -165,6 +165,24 @@ int adsc_get_fields_host_async(adsc_handle h, double *h_Phi, double *h_Pi, doubl
  * stream.  EINVAL for J outside 1..32 or a NULL pointer, ESTATE before adsc_set_initial. */
 int adsc_mode_energies(adsc_handle h, int J, double *host_out);
 
+/* Roofline denominators measured on the current CUDA device ("a DFMA issue-rate probe and a
+ * shared-memory bandwidth probe"; none of the method's arithmetic).  kind ADSC_PROBE_FP64_FMA: *result = flop/s of
+ * independent FP64 fused multiply-adds on every SM (2 flop each); ADSC_PROBE_SHARED_LOAD: *result = bytes/s of
+ * conflict-free 128-bit shared-memory loads on every SM.  Runs its own kernel for about target_ms milliseconds on a
+ * private stream and synchronises; needs no handle.  result is a HOST pointer.  EINVAL on bad arguments, ECUDA
+ * without a device. */
+#define ADSC_PROBE_FP64_FMA    0
+#define ADSC_PROBE_SHARED_LOAD 1
+int adsc_probe(int kind, double target_ms, double *result);
+
+/* Self-test of the one transcendental on the hot path (e^{-delta} of eqs (2), (3)): evaluates the
+ * kernels' own exponential routine on ngroups groups of 8 arguments (h_x[8*g .. 8*g+7], the 8 points one thread
+ * owns; the last one is the group's reference point) and returns the results h_E[8*ngroups] and, per group, which
+ * evaluation the routine chose: h_tier[g] = 0, 1, 2 for the relative polynomial with 2, 3, 5 terms (largest
+ * |x_p - x_7| <= 2^-14, 2^-10, 2^-6), 3 for one full evaluation per point.  HOST pointers, owned by the caller;
+ * synchronous; allocates and frees its own device scratch.  EINVAL on bad arguments, ECUDA without a device. */
+int adsc_selftest_exp(int ngroups, const double *h_x, double *h_E, int *h_tier);
+
 /* Number of kernels this handle has launched since adsc_bind (for gpu_launches). */
 long long adsc_launch_count(adsc_handle h);
 

@@ -23,6 +23,7 @@ ADSC_OPT_STEPS_PER_LAUNCH = 4
 ADSC_OPT_FIXED_BACKGROUND = 7
 ADSC_OPT_RK_ORDER = 8
 PATH_AUTO, PATH_STREAM, PATH_RESIDENT = 0, 1, 2
+ADSC_PROBE_FP64_FMA, ADSC_PROBE_SHARED_LOAD = 0, 1
 
 
 class adsc_diag(C.Structure):
@@ -64,6 +65,8 @@ _SIGS = {
     "adsc_launch_count": (C.c_longlong, [C.c_void_p]),
     "adsc_path": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
     "adsc_last_error": (C.c_char_p, [C.c_void_p]),
+    "adsc_selftest_exp": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "adsc_probe": (C.c_int, [C.c_int, C.c_double, C.POINTER(C.c_double)]),
 }
 
 
@@ -164,6 +167,27 @@ def adsc_path(h):
     cl = C.c_int(0)
     p = load_library().adsc_path(h, C.byref(cl))
     return p, cl.value
+
+
+def adsc_selftest_exp(x):
+    """x: float64 [ngroups][8].  Returns (E [ngroups][8], tier [ngroups]) from the kernels' own exponential."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    assert x.ndim == 2 and x.shape[1] == 8
+    E = np.empty_like(x)
+    tier = np.empty(x.shape[0], dtype=np.int32)
+    code = load_library().adsc_selftest_exp(x.shape[0], x.ctypes.data, E.ctypes.data, tier.ctypes.data)
+    if code != ADSC_OK:
+        raise AdscError(code, "adsc_selftest_exp failed")
+    return E, tier
+
+
+def adsc_probe(kind, target_ms=50.0):
+    """flop/s (ADSC_PROBE_FP64_FMA) or bytes/s (ADSC_PROBE_SHARED_LOAD) measured on the current CUDA device."""
+    out = C.c_double(0.0)
+    code = load_library().adsc_probe(int(kind), float(target_ms), C.byref(out))
+    if code != ADSC_OK:
+        raise AdscError(code, "adsc_probe failed (no CUDA device?)")
+    return out.value
 
 
 # ------------------------------------------------------------------ convenience wrapper

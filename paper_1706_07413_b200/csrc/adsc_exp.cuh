@@ -45,8 +45,9 @@ __device__ __forceinline__ double exp3_ref(double x)
 // relative to it.  exp(z) = 1 + z t(z), t = sum_{k<=5} z^k/(k+1)!; for |z| <= 2^-6 the truncation
 // is z^7/5040 < 5e-17 relative.  x = 0 gives exactly 1 (pure AdS stays bit-exact).
 // `scale` multiplies every result (one extra multiplication: it is folded into the reference value).
+// tier (self-test only): 0, 1, 2 = 2, 3, 5 terms of t; 3 = a full evaluation per point.
 template <int P, bool SCALED = false>
-__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], const double scale = 1.0)
+__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], const double scale = 1.0, int *tier = nullptr)
 {
     const double xr = x[P - 1];
     double z[P];
@@ -61,6 +62,7 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], 
     }
     const double Er = SCALED ? exp3_ref(xr) * scale : exp3_ref(xr);
     E[P - 1] = Er;
+    if (tier) *tier = sml + mid + big;       // which branch below runs (adsc_selftest_exp only; folds away otherwise)
     if (!sml) {                              // |z| <= 2^-14: two terms of t suffice (z^4/24 < 6e-19)
 #pragma unroll
         for (int p = 0; p < P - 1; ++p) {

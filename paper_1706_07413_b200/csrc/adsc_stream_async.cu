@@ -44,6 +44,10 @@ constexpr int SA_TS = 4 * SA_RS;          // tile stride
 constexpr int SA_FS = 3 * SA_TS + 4 * SA_RS3;   // field stride (16-byte units)
 constexpr int SA_MBOX = 40;               // doubles per chunk mailbox: 17 slots {value, stamp} + padding
 constexpr int SA_SLOT = SA_SL * 8;        // bytes of one table slice
+// The two warps with the fewest slices of a ragged chunk serve the stage: SA_WS scans the slice totals, publishes the
+// chunk total and computes the boundary fluxes (pre-pass); SA_WH exchanges the chunk edges and later gathers the
+// totals of the other chunks.  In the top (ragged) tile, which a stage processes first, they are the idle ones.
+constexpr int SA_WS = SA_NW - 1, SA_WH = SA_NW - 2;
 
 // shared-memory map (bytes)
 constexpr int SA_OFF_RING = 3 * SA_FS * 16;
@@ -61,8 +65,8 @@ constexpr int o_xa = o_xh + 16;           // [4] A at the two points below / abo
 constexpr int o_esc = o_xa + 4;           // [28][2] -2 sc just below / just above every slice
 constexpr int o_etab = o_esc + 2 * SA_MAXQ;   // [5][6] tables around every boundary the pre-pass serves
 constexpr int o_scal = o_etab + 32;       // [8] scalars: 0 collapse flag of the member, 1 factor C of the chunks above
-constexpr int o_mbar = o_scal + 8;        // mbF, ring[8][3]
-constexpr int SA_MISC_DOUBLES = o_mbar + 26;
+constexpr int o_mbar = o_scal + 8;        // mbF, ring[8][3], mbC, mbB
+constexpr int SA_MISC_DOUBLES = o_mbar + 28;
 constexpr size_t SA_SMEM = (size_t)SA_OFF_MISC + (size_t)SA_MISC_DOUBLES * 8;
 static_assert(SA_SMEM <= 232448, "shared memory of the streaming kernel");
 static_assert(o_flo % 2 == 0 && o_fhi % 2 == 0 && o_fpre % 2 == 0 && o_ftop % 2 == 0 && o_xh % 2 == 0, "16-byte slots");
@@ -171,12 +175,14 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     const uint32_t mbF = smem_u32(misc + o_mbar);
     const uint32_t mbR = mbF + 8 + (uint32_t)warp * 24;  // this warp's three ring barriers
     const uint32_t mbC = mbF + 8 * 25;                   // "the factor of the chunks above is in shared memory"
+    const uint32_t mbB = mbF + 8 * 26;                   // "slice bases and chunk halos are in shared memory"
     const uint32_t ringw = smem_u32(smraw + SA_OFF_RING) + (uint32_t)warp * 3 * SA_SLOT;
     const double2 *slot = reinterpret_cast<const double2 *>(smraw + SA_OFF_RING + (size_t)warp * 3 * SA_SLOT);
     if (tid == 0) {
         mbar_init(mbF, SA_NW);
         for (int k = 0; k < 3 * SA_NW; ++k) mbar_init(mbF + 8 + 8 * k, 1);
         mbar_init(mbC, 1);
+        mbar_init(mbB, 2);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // columns of threads that own no point are read as halos by their neighbours: keep them finite
@@ -310,7 +316,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                 const int par = (int)(stage_ctr & 1u);                   // mailbox buffer of this round
                 ++stage_ctr;
                 __syncthreads();                                         // S1: state, slice totals, flags of every tile
-                if (warp == 0) {
+                if (warp == SA_WS) {
                     // ---- a2, slice level: exclusive suffix over the chunk's slices; the chunk total (with the collapse
                     // flag in the low bit of its stamp) goes to the chunk's mailbox.  Every 16-byte mailbox slot is
                     // {value, stamp of the round}: one 128-bit store / load each, no fence, no counter, no atomics.
@@ -326,7 +332,8 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         if (lane == 0) st_pair(mine, incl, 2ULL * stage_ctr + (anyf ? 1ULL : 0ULL));
                         if (lane < NQ) base[lane] = exq;                   // within the chunk (see `gather`)
                     }
-                    asm volatile("bar.sync 1, 64;" ::: "memory");        // the chunk halos (warp 1) are in shared memory
+                    warp_arrive(mbB);
+                    asm volatile("bar.sync 1, 64;" ::: "memory");        // the chunk halos (warp SA_WH) are in shared memory
                     // ---- pre-pass: fluxes at the two points below every tile of the chunk and above the chunk, which
                     // the owner computes later in this stage or in another CTA (one lane per point, full exponential)
                     if (lane < 10) {
@@ -364,7 +371,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             dst[2 + e] = etab[6 * m + 4 + e] * Gv;
                         }
                     }
-                } else if (warp == 1) {
+                } else if (warp == SA_WH) {
                     // ---- state edges of the chunk to its mailbox; halo columns at the tile boundaries inside the chunk
                     // (the tile below a boundary is full); the neighbours' edges, or the parity ghosts, to shared memory
                     double *mbx = prm.mbox + (size_t)gi * 2 * G * SA_MBOX;
@@ -402,14 +409,18 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         if (f == 2) xa[2 * up + off] = v;
                         else xh[8 * up + 4 * f + (up ? 0 : 1) + off] = v;
                     }
+                    warp_arrive(mbB);
                     asm volatile("bar.sync 1, 64;" ::: "memory");
                 }
-                __syncthreads();                                         // S2
+                // S2: bases (SA_WS) and halos (SA_WH) are there.  The pre-pass of SA_WS runs on beside the first tile:
+                // its results are read in phase 2, behind the tile's sync F, on which SA_WS arrives after the pre-pass;
+                // it reads the state of tiles that nobody changes before that sync.
+                mbar_wait<false>(mbB, (uint32_t)par);    // one phase per barrier round: its parity is the mailbox parity
                 if (s == 0 && n == prm.nsteps) {                         // final flag round only: nothing to overlap
                     if constexpr (!FIXED) {
                         const uint32_t cpar = (phs >> 4) & 1u;
                         phs ^= 16u;
-                        if (warp == SA_NW - 1) gather(par);
+                        if (warp == SA_WH) gather(par);
                         mbar_wait<false>(mbC, cpar);
                         // a6: collapse test of PAPER.md:85 on the state after n steps (flags of every chunk)
                         if (n > 0 && scal[0] != 0.0) collapsed = 1;
@@ -426,7 +437,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     const bool defer = !FIXED && (j == NT - 1);
                     if (j >= n_my) {                                      // ragged top tile: nothing to do for this warp
                         if (defer) {
-                            if (warp == SA_NW - 1) gather(par);
+                            if (warp == SA_WH) gather(par);
                             mbar_wait<false>(mbC, cpar);
                             Cst = scal[1];
                             if (s == 0 && n > 0 && scal[0] != 0.0) { collapsed = 1; break; }     // a6
@@ -573,7 +584,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     }
                     if (first) kAv[0] = 0.0;                                      // A(0,t)=1, eq (8)
                     if (defer) {
-                        if (warp == SA_NW - 1) gather(par);
+                        if (warp == SA_WH) gather(par);
                         mbar_wait<false>(mbC, cpar);
                         Cst = scal[1];
                         if (s == 0 && n > 0 && scal[0] != 0.0) {                  // a6: nothing has been changed yet

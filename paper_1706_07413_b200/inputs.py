@@ -12,6 +12,7 @@ Workloads (BASELINE.json configs; recipe in DESIGN.md "Input recipe"):
   cfg4  N=2^20+1 B=1     Gaussian Pi, sigma=1/16, eps=1
   cfg5  N=2049  B=16384  Gaussian Pi, sigma~U[0.2,0.5], eps~U[0.05,0.5]
   tcollapse N=1025 B=64  Gaussian Pi, sigma=1/16, eps~U[30,60] (test only)
+  paper32k N=2^15+1 B=64 eq (13) family k_d=3, mu=1, one member per amplitude (the paper's production shape)
 The paper's own initial data are mode sums with Phi(x,0)=0 (PAPER.md:89-93,
 111); no public dataset is involved, these seeded ensembles stand in.  qp_family()
 generates the paper's families themselves (eq (13)) for the t_c(eps) driver.
@@ -121,6 +122,8 @@ def two_mode(N: int, a_tot, ratio, theta1):
     return Phi, Pi
 
 
+PAPER32K_EPS = (0.02, 0.08)       # amplitude range of the paper32k ensemble (smallest, largest)
+
 CONFIGS = {
     # name: (N, B, steps, courant, ko_eps)
     "cfg1": dict(N=1025, B=1, steps=26076, idx=1),
@@ -129,11 +132,14 @@ CONFIGS = {
     "cfg4": dict(N=2 ** 20 + 1, B=1, steps=1000, idx=4),
     "cfg5": dict(N=2049, B=16384, steps=2607595, idx=5),
     "tcollapse": dict(N=1025, B=64, steps=10431, idx=6),
+    # the paper's production shape: 2^15 points, RK3, one member per amplitude of the
+    # k_d = 3, mu = 1 family of eq (13); the amplitudes are ours (the paper prints none), equally spaced in 1/eps^2
+    "paper32k": dict(N=2 ** 15 + 1, B=64, steps=41721513, idx=7),
 }
 
 
-def make(name: str, B: int | None = None, N: int | None = None):
-    """(Phi, Pi, params) for a named workload, first B members (default all).
+def make(name: str, B: int | None = None, N: int | None = None, lo: int = 0):
+    """(Phi, Pi, params) for a named workload, members [lo, B) of the (tiled) ensemble (default all).
     seed = 170607413 + config index; same arrays feed oracle and GPU."""
     cfg = CONFIGS[name]
     N = N or cfg["N"]
@@ -148,15 +154,22 @@ def make(name: str, B: int | None = None, N: int | None = None):
         sig = rng.uniform(0.2, 0.5, Bfull); eps = rng.uniform(0.05, 0.5, Bfull)
     elif name == "tcollapse":
         eps = rng.uniform(30.0, 60.0, Bfull); sig = np.full(Bfull, 1.0 / 16)
+    elif name == "paper32k":
+        inv2 = np.linspace(1.0 / PAPER32K_EPS[1] ** 2, 1.0 / PAPER32K_EPS[0] ** 2, Bfull)
+        eps = 1.0 / np.sqrt(inv2)
+        reps = -(-B // Bfull)
+        eps = np.tile(eps, reps)[lo:B]
+        Phi, Pi, _ = qp_family(N, eps, mu=1.0, kd=3)
+        return Phi, Pi, dict(eps=eps, mu=1.0, kd=3)
     elif name == "cfg3":
         a = rng.uniform(0.01, 0.1, Bfull); r = rng.uniform(0.2, 1.0, Bfull)
         th = rng.uniform(0.0, 2 * np.pi, Bfull)
         reps = -(-B // Bfull)
-        a, r, th = (np.tile(v, reps)[:B] for v in (a, r, th))
+        a, r, th = (np.tile(v, reps)[lo:B] for v in (a, r, th))
         Phi, Pi = two_mode(N, a, r, th)
         return Phi, Pi, dict(a_tot=a, ratio=r, theta1=th)
     reps = -(-B // Bfull)
-    eps, sig = np.tile(eps, reps)[:B], np.tile(sig, reps)[:B]
+    eps, sig = np.tile(eps, reps)[lo:B], np.tile(sig, reps)[lo:B]
     Pi = gaussian_Pi(N, eps, sig)
     Phi = np.zeros_like(Pi)
     return Phi, Pi, dict(eps=eps, sigma=sig)

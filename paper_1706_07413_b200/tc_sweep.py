@@ -16,14 +16,16 @@ import numpy as np
 
 
 def sweep(eps, mu: float, kd: int, N: int = 4097, tmax: float = 500.0, threshold: float = 0.01,
-          courant: float = 0.25, ko_eps: float = 0.1, chunk_steps: int = 2000, device: str = "cuda:0"):
+          courant: float = 0.25, ko_eps: float = 0.1, chunk_steps: int = 2000, device: str = "cuda:0",
+          rk_order: int = 4):
     """Returns a dict of arrays over the amplitudes: eps, t_collapse (NaN if none by t_max), collapsed,
     t (time reached), mass0, mass, mass_loss, min_A."""
     import torch
     from . import binding, inputs
     eps = np.atleast_1d(np.asarray(eps, dtype=np.float64))
     Phi, Pi, _ = inputs.qp_family(N, eps, mu, kd)
-    ens = binding.Ensemble(N, len(eps), courant=courant, ko_eps=ko_eps, device=device, threshold=threshold)
+    ens = binding.Ensemble(N, len(eps), courant=courant, ko_eps=ko_eps, device=device, threshold=threshold,
+                           rk_order=(rk_order if rk_order != 4 else None))
     ens.set_initial(torch.from_numpy(Phi).to(device), torch.from_numpy(Pi).to(device))
     d0 = ens.diagnostics()
     nsteps = int(np.ceil(tmax / ens.dt))            # reading R18
@@ -38,6 +40,7 @@ def sweep(eps, mu: float, kd: int, N: int = 4097, tmax: float = 500.0, threshold
             break
     out = dict(eps=eps, t_collapse=d["t_collapse"].copy(), collapsed=d["collapsed"].copy(), t=d["t"].copy(),
                mass0=d0["mass"].copy(), mass=d["mass"].copy(), min_A=d["min_A"].copy())
+    out["path"] = ens.path
     out["mass_loss"] = np.abs(out["mass"] - out["mass0"]) / np.abs(out["mass0"])
     ens.close()
     return out
@@ -51,10 +54,13 @@ def main(argv=None):
     ap.add_argument("--N", type=int, default=4097)
     ap.add_argument("--tmax", type=float, default=50.0)
     ap.add_argument("--threshold", type=float, default=0.01, help="collapse when min A < this (PAPER.md:85)")
+    ap.add_argument("--rk-order", type=int, default=4, choices=[2, 3, 4], help="the paper's production runs used 3 (PAPER.md:57)")
+    ap.add_argument("--chunk-steps", type=int, default=2000, help="RK steps between two looks at the collapse flags")
     a = ap.parse_args(argv)
     eps = [float(v) for v in a.eps.split(",")]
-    r = sweep(eps, a.mu, a.kd, N=a.N, tmax=a.tmax, threshold=a.threshold)
-    print(f"# family k_d={a.kd} mu={a.mu} N={a.N} t_max={a.tmax} threshold={a.threshold}")
+    r = sweep(eps, a.mu, a.kd, N=a.N, tmax=a.tmax, threshold=a.threshold, rk_order=a.rk_order, chunk_steps=a.chunk_steps)
+    print(f"# family k_d={a.kd} mu={a.mu} N={a.N} t_max={a.tmax} threshold={a.threshold} rk_order={a.rk_order} "
+          f"path={r['path'][0]} ctas_per_member={r['path'][1]}")
     print("# eps        1/eps^2      t_collapse   t_reached    mass_loss    min_A")
     for i in range(len(eps)):
         print(f"{r['eps'][i]:10.4e} {1.0 / r['eps'][i] ** 2:12.4e} {r['t_collapse'][i]:12.5f} {r['t'][i]:12.5f} "

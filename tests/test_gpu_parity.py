@@ -460,3 +460,116 @@ def test_pipelined_ensemble_equals_single_handle(env):
         assert np.array_equal(out[k].numpy(), ref[k]), k
     assert (d["steps_done"] == 150).all() and np.array_equal(d["mass"], dref["mass"])
     pe.close()
+
+
+# ------------------------------------------------- round-2 additions: holes named by the round-1 review
+
+@pytest.mark.parametrize("path", [2, 1, 3])
+def test_strong_field_1000_steps_absolute(env, path):
+    """A member on its way to collapse (eps = 40, 38, sigma = 1/16, N = 1025; no collapse within 1000 steps, min A
+    falls to 0.74) at the [NS] tolerance, ABSOLUTE, in all four fields including delta.  This is the regime where a
+    thread's eight exponents differ by more than 2^-6 (delta changes by 0.1 - 0.2 over 8 points: full evaluations,
+    adsc_exp.cuh)."""
+    Pi = env["inputs"].gaussian_Pi(1025, [40.0, 38.0], [1.0 / 16, 1.0 / 16])
+    Phi = np.zeros_like(Pi)
+    ens, f, d = _gpu_run(env, Phi, Pi, 1000, path=path)
+    assert ens.path[0] == path
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=2).step(1000)
+    assert (ev.diagnostics()["collapsed"] == 0).all() and (d["collapsed"] == 0).all()
+    assert np.abs(ev.delta[:, :-7] - ev.delta[:, 7:]).max() > 4 * 2.0 ** -6 and ev.A.min() < 0.8
+    _compare(f, ev)
+    _bc_invariants(f)
+
+
+def test_exp_tiers_exercised_and_accurate(env):
+    """Directed test of the hot path's exponential (adsc_selftest_exp): every branch of exp3_near is taken for the
+    spread it is meant for, and every result is within 2 ulp of e^x (x87 long double as the reference)."""
+    binding = env["binding"]
+    rng = np.random.default_rng(11)
+    groups, want = [], []
+    for tier, (lo, hi) in enumerate(((0.0, 2.0 ** -14), (2.0 ** -14, 2.0 ** -10), (2.0 ** -10, 2.0 ** -6), (2.0 ** -6, 3.0))):
+        for _ in range(4000):
+            xr = rng.uniform(-30.0, 2.0)
+            z = rng.uniform(-hi, hi, 7)
+            k = rng.integers(0, 7)
+            z[k] = np.sign(z[k] if z[k] != 0 else 1.0) * rng.uniform(max(lo * 1.001, 0.0), hi * 0.999)   # the spread that selects the tier
+            if tier == 0 and rng.uniform() < 0.1:
+                z[:] = 0.0
+            groups.append(np.concatenate([xr + z, [xr]]))
+            want.append(tier)
+    x = np.array(groups)
+    # the tier is decided from the rounded differences x_p - x_7: recompute them as the kernel does
+    zmax = np.abs(x[:, :7] - x[:, 7:8]).max(axis=1)
+    want = np.where(zmax > 2.0 ** -6 * (1 + 2.0 ** -19), 3, np.where(zmax > 2.0 ** -10 * (1 + 2.0 ** -19), 2,
+                    np.where(zmax > 2.0 ** -14 * (1 + 2.0 ** -19), 1, 0)))
+    E, tier = binding.adsc_selftest_exp(x)
+    assert np.array_equal(tier, want)
+    for t in range(4):
+        assert (tier == t).sum() >= 3000
+    ref = np.exp(x.astype(np.longdouble))
+    ulp = np.spacing(ref.astype(np.float64))
+    err = np.abs((E.astype(np.longdouble) - ref) / ulp).astype(np.float64)
+    assert err.max() <= 2.0, err.max()
+    one, t0 = binding.adsc_selftest_exp(np.zeros((1, 8)))
+    assert (one == 1.0).all() and t0[0] == 0                      # e^0 = 1 exactly (pure AdS)
+
+
+@pytest.mark.parametrize("name,B,nsteps", [("cfg2", 160, 50), ("cfg5", 330, 50), ("cfg3", 40, 30)])
+def test_more_members_than_one_wave(env, name, B, nsteps):
+    """Resident path with more members than co-resident clusters (74 clusters of 2, 148 single CTAs, 33 clusters of
+    4): CTAs of a second wave start on SMs whose shared memory and mbarriers a first-wave CTA has used."""
+    Phi, Pi, _ = env["inputs"].make(name, B=B)
+    ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=2)
+    assert ens.path[0] == 2 and B * ens.path[1] > 148
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=16).step(nsteps)
+    _compare(f, ev)
+    _bc_invariants(f)
+    assert (d["steps_done"] == nsteps).all() and (d["collapsed"] == 0).all()
+
+
+@pytest.mark.parametrize("path", [2, 1, 3])
+@pytest.mark.parametrize("K_A", [1, 7])
+def test_collapse_with_A_resolve_period(env, path, K_A):
+    """Collapse detected on and between the K_A boundaries (A re-solved from eq (5) every K_A steps),
+    in one adsc_step call and with steps_per_launch splitting the launches: flags, collapse times and step counts
+    as the oracle's."""
+    B, nsteps = 8, 3300
+    Phi, Pi, _ = env["inputs"].make("tcollapse", B=B)
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=8, K_A=K_A).step(nsteps)
+    od = ev.diagnostics()
+    assert od["collapsed"].any() and not od["collapsed"].all()
+    for spl in (None, 50):
+        ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=path, a_resolve_period=K_A, steps_per_launch=spl)
+        assert ens.path[0] == path
+        assert (d["collapsed"] == od["collapsed"]).all()
+        for b in range(B):
+            if od["collapsed"][b]:
+                assert abs(d["t_collapse"][b] - od["t_collapse"][b]) <= ev.dt * (1 + 1e-12)
+                assert abs(d["steps_done"][b] - od["steps_done"][b]) <= 1
+            else:
+                assert d["steps_done"][b] == nsteps and np.isnan(d["t_collapse"][b])
+
+
+SANITIZER_CASES = [
+    # (N, B, path, kw): one launch of every stage-kernel family and cluster size, 3 steps
+    (17, 2, 3, {}), (33, 2, 1, {}), (33, 2, 3, {}), (129, 2, 2, {}), (1025, 2, 2, {}), (1025, 2, 1, {}),
+    (2049, 2, 2, {}), (3073, 2, 0, {}), (4097, 2, 2, {}), (8193, 2, 2, {}), (16385, 1, 2, {}),
+    (20481, 3, 1, {}), (4097, 2, 2, dict(rk_order=3)), (2049, 2, 2, dict(fixed_background=True)),
+    (20481, 2, 1, dict(fixed_background=True)),
+]
+
+
+@pytest.mark.parametrize("N,B,path,kw", SANITIZER_CASES)
+def test_short_runs_every_kernel_family(env, N, B, path, kw):
+    """Three steps of every stage-kernel family against the oracle.  This is also the command that is run under
+    compute-sanitizer (memcheck, racecheck, synccheck, initcheck; profiles/r02_sanitizer.md)."""
+    Phi, Pi, _ = env["inputs"].make("cfg5", B=B, N=N)
+    Pi = Pi * 4.0
+    ens, f, d = _gpu_run(env, Phi, Pi, 3, path=path, **kw)
+    okw = dict(fixed_background=True) if kw.get("fixed_background") else {}
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=2, rk_order=kw.get("rk_order", 4), **okw).step(3)
+    if kw.get("fixed_background"):
+        assert np.max(np.abs(f["Phi"] - ev.Phi)) <= TOL and np.max(np.abs(f["Pi"] - ev.Pi)) <= TOL
+    else:
+        _compare(f, ev)
+    assert (d["steps_done"] == 3).all()
