@@ -70,6 +70,9 @@ def parse():
     ap.add_argument("--e2e-parts", type=int, default=8, help="sub-batches (handles, streams) of the e2e leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--mode-energies", type=int, default=0, metavar="J",
+                    help="also time adsc_mode_energies(J) (SURVEY.md 8(f) f3) on the evolved ensemble and add a "
+                         "`mode_energies` object with its own roofline to the line")
     ap.add_argument("--probe-ms", type=float, default=50.0, help="duration of each roofline-denominator probe (0 = skip)")
     a = ap.parse_args()
     if a.rk_order == 0:
@@ -300,6 +303,23 @@ def main():
     updates = (n_active if args.masked_fraction > 0.0 else float(B) * world) * N * rk4 * K
     value = updates / (ms * 1e-3)
 
+    # ---- f3: normal-mode projection of the evolved ensemble (off the per-step path; its own roofline)
+    modes = None
+    if args.mode_energies > 0:
+        J = args.mode_energies
+        ens.mode_energies(J)                               # warm-up
+        torch.cuda.synchronize(dev)
+        tm0 = time.perf_counter()
+        reps = 5
+        for _ in range(reps):
+            ens.mode_energies(J)                           # two kernels + D2H of [B][J]; synchronises
+        tm = (time.perf_counter() - tm0) / reps
+        # per point: sincospi and the j-independent weights (~45 FP64-pipe instr), per point and mode: two Jacobi
+        # recurrences (6) + two projections (4)
+        m_slots = 45.0 + 10.0 * J
+        modes = {"J": J, "ms_per_call": tm * 1e3, "points_per_s": B * N / tm, "algorithmic": f"{m_slots:.0f} FP64-pipe instr per point",
+                 "achieved_tflops": B * N / tm * m_slots * 2 / 1e12}
+
     # ---- end to end through the C ABI with HOST buffers: H2D of Phi, Pi + step + D2H of the fields
     Phi_o = torch.empty_like(Phi_h).pin_memory(); Pi_o = torch.empty_like(Phi_h).pin_memory()
     A_o = torch.empty_like(Phi_h).pin_memory()
@@ -408,6 +428,10 @@ def main():
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if modes is not None:
+        modes["roofline"] = {"bound": "alu", "achieved": modes.pop("achieved_tflops"), "peak": peak_tf, "unit": "TFLOP/s"}
+        modes["roofline"]["frac"] = modes["roofline"]["achieved"] / peak_tf
+        line["mode_energies"] = modes
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -161,8 +161,9 @@ int adsc_get_fields_host_async(adsc_handle h, double *h_Phi, double *h_Pi, doubl
  * decomposed into a spectrum of normal modes").  For the AdS4 modes e_j (R19),
  * j < J <= 32: Pi_j = int Pi e_j tan^2 x dx, Phi_j = int Phi e_j' tan^2 x dx (composite Simpson, integrand 0
  * at x = pi/2), E_j = Pi_j^2 + Phi_j^2 / omega_j^2, omega_j = 3 + 2j (R24).  host_out: HOST array
- * [batch][J], row-major, owned by the caller.  One kernel launch plus one small D2H copy; synchronises the
- * stream.  EINVAL for J outside 1..32 or a NULL pointer, ESTATE before adsc_set_initial. */
+ * [batch][J], row-major, owned by the caller.  Two kernel launches (slice partials over several CTAs per member,
+ * then a fixed-order sum) plus one small D2H copy; synchronises the stream.  EINVAL for J outside 1..32, J > N/4
+ * or a NULL pointer, ESTATE before adsc_set_initial. */
 int adsc_mode_energies(adsc_handle h, int J, double *host_out);
 
 /* Roofline denominators measured on the current CUDA device ("a DFMA issue-rate probe and a

@@ -2,6 +2,7 @@
 
 `python -m paper_1706_07413_b200.build [--force]` or `build()` from Python.  The
 library links only against the CUDA runtime (statically), so it loads without torch.
+ADSC_NVCC_EXTRA (environment) adds nvcc flags, e.g. the -D tuning macros the kernels document.
 """
 from __future__ import annotations
 
@@ -52,7 +53,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for src in sources():
         obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
         objs.append(obj)
-        cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-c", src, "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("ADSC_NVCC_EXTRA", "").split(), "-I", INCLUDE, "-c", src, "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((cmd, subprocess.Popen(cmd)))

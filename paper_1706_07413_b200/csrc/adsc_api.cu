@@ -174,7 +174,7 @@ int adsc_set_option(adsc_handle h, int key, double value)
         if (!(value == 2.0 || value == 3.0 || value == 4.0)) return fail(h, ADSC_EINVAL, "Runge-Kutta order: 2, 3 or 4");
         if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_RK_ORDER before adsc_bind");
         h->rk_order = (int)value;
-        resolve_path(h);                 // (generation-1 and tuning configurations of the resident kernel are RK4 only)
+        resolve_path(h);                 // (the fixed-background build of the resident kernel is RK4 only)
         if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
         return ADSC_OK;
     default:
@@ -225,6 +225,19 @@ int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream)
         int G = 0, SQ = 0, groups = 0;
         if (!stream_async_select(h->pb.N, h->pb.B, h->dev_sms, &G, &SQ, &groups) || sa_row_pitch(h->pb.N, G, SQ) != h->pb.NP) { h->path = 3; h->sp_ok = false; }
         else { h->sp_G = G; h->sp_SQ = SQ; h->sp_groups = groups; }
+    }
+    // the resident configuration was chosen at adsc_create without a device: make sure THIS device can hold one
+    // cluster of it (shared-memory opt-in, cluster size)
+    if (h->path == 2) {
+        int clusters = 0;
+        const cudaError_t e = resident_check(h, &clusters);
+        if (e != cudaSuccess || clusters < 1) {
+            (void)cudaGetLastError();
+            return fail(h, ADSC_ECUDA, std::string("the resident kernel (") + resident_cfg_name(h->res_cfg) + ", "
+                        + std::to_string(h->cluster) + " CTAs per member) cannot run on this device"
+                        + (e != cudaSuccess ? std::string(": ") + cudaGetErrorString(e) : std::string())
+                        + "; set ADSC_OPT_PATH to 1 (streaming) before adsc_bind");
+        }
     }
     const size_t NT = (size_t)h->pb.NP + 2 * HAL;
     h->tb.sc = h->ws.tab + 0 * NT + HAL;
@@ -392,9 +405,10 @@ int adsc_mode_energies(adsc_handle h, int J, double *host_out)
     if (!h) return fail(nullptr, ADSC_EINVAL, "null handle");
     if (!h->bound || !h->have_state) return fail(h, ADSC_ESTATE, "adsc_bind and adsc_set_initial first");
     if (!host_out) return fail(h, ADSC_EINVAL, "null output");
-    if (J < 1 || J > 32 || J > h->pb.NP) return fail(h, ADSC_EINVAL, "J must be in 1..32 (and <= N)");
-    double *d_out = h->ws.Ac;                    // scratch: [B][NP] doubles, enough for [B][J]
-    ADSC_CUDA(launch_mode_energies(h, J, d_out), "mode projection kernel");
+    if (J < 1 || J > 32 || 4 * J > h->pb.NP) return fail(h, ADSC_EINVAL, "J must be in 1..32 (and <= N/4)");
+    double *d_out = h->ws.Ac;                    // scratch: [B][NP] doubles: [B][J] results, then the slice partials
+    const size_t used = ((size_t)h->pb.B * J + 31) / 32 * 32;
+    ADSC_CUDA(launch_mode_energies(h, J, d_out, d_out + used, (size_t)h->pb.B * h->pb.NP - used), "mode projection kernels");
     ADSC_CUDA(cudaMemcpyAsync(host_out, d_out, (size_t)h->pb.B * J * sizeof(double), cudaMemcpyDeviceToHost, h->stream),
               "D2H mode energies");
     ADSC_CUDA(cudaStreamSynchronize(h->stream), "stream synchronize");

@@ -45,9 +45,13 @@ __device__ __forceinline__ double exp3_ref(double x)
 // relative to it.  exp(z) = 1 + z t(z), t = sum_{k<=5} z^k/(k+1)!; for |z| <= 2^-6 the truncation
 // is z^7/5040 < 5e-17 relative.  x = 0 gives exactly 1 (pure AdS stays bit-exact).
 // `scale` multiplies every result (one extra multiplication: it is folded into the reference value).
+// SHIFTED: every argument is x_p + shift; the differences do not contain the shift, so it is added to the
+// reference argument only (and to every argument if full evaluations are needed) -- the caller may have `shift`
+// ready much later than x.
 // tier (self-test only): 0, 1, 2 = 2, 3, 5 terms of t; 3 = a full evaluation per point.
-template <int P, bool SCALED = false>
-__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], const double scale = 1.0, int *tier = nullptr)
+template <int P, bool SCALED = false, bool SHIFTED = false>
+__device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], const double scale = 1.0, int *tier = nullptr,
+                                          const double shift = 0.0)
 {
     const double xr = x[P - 1];
     double z[P];
@@ -60,7 +64,8 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], 
         mid |= (hz > 0x3f500000) ? 1 : 0;    // |z| > 2^-10
         sml |= (hz > 0x3f100000) ? 1 : 0;    // |z| > 2^-14
     }
-    const double Er = SCALED ? exp3_ref(xr) * scale : exp3_ref(xr);
+    const double xs = SHIFTED ? xr + shift : xr;
+    const double Er = SCALED ? exp3_ref(xs) * scale : exp3_ref(xs);
     E[P - 1] = Er;
     if (tier) *tier = sml + mid + big;       // which branch below runs (adsc_selftest_exp only; folds away otherwise)
     if (!sml) {                              // |z| <= 2^-14: two terms of t suffice (z^4/24 < 6e-19)
@@ -90,7 +95,10 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], 
         }
     } else {
 #pragma unroll
-        for (int p = 0; p < P - 1; ++p) E[p] = SCALED ? exp3_ref(x[p]) * scale : exp3_ref(x[p]);
+        for (int p = 0; p < P - 1; ++p) {
+            const double xp = SHIFTED ? x[p] + shift : x[p];
+            E[p] = SCALED ? exp3_ref(xp) * scale : exp3_ref(xp);
+        }
     }
 }
 

@@ -124,7 +124,8 @@ cudaError_t launch_solve(adsc_ctx *c, int mode);              // one CTA per mem
 cudaError_t launch_solve_tiled(adsc_ctx *c, int mode);        // adsc_solve_tiled.cu (streaming layouts only)
 constexpr int SOLVE_TILED_MIN_N = 32768;                      // members at least this long use the tiled solve
 cudaError_t launch_finalize(adsc_ctx *c, int inc_steps);
-cudaError_t launch_mode_energies(adsc_ctx *c, int J, double *d_out);   // adsc_modes.cu; d_out [B][J]
+// adsc_modes.cu; d_out [B][J]; scratch for the slice partials (at least 2 B J doubles)
+cudaError_t launch_mode_energies(adsc_ctx *c, int J, double *d_out, double *scratch, size_t scratch_doubles);
 cudaError_t launch_stream_step(adsc_ctx *c);                 // one RK4 step, generic streaming kernels
 // persistent streaming kernel (adsc_stream_async.cu): chunks per member, slices per chunk, concurrent members
 bool stream_async_select(int N, int B, int sms, int *G, int *SQ, int *groups);
@@ -132,6 +133,7 @@ cudaError_t launch_tabp(adsc_ctx *c);                        // permuted coeffic
 cudaError_t launch_stream_async(adsc_ctx *c, long long nsteps, int check_last);
 cudaError_t launch_resident(adsc_ctx *c, long long nsteps, int check_last);  // resident path
 bool resident_select(adsc_ctx *c);                           // fills c->cluster, c->res_cfg
+cudaError_t resident_check(adsc_ctx *c, int *clusters);      // at adsc_bind: clusters of the selected kernel the device holds at once
 const char *resident_cfg_name(int cfg);
 
 // ---- device helpers ----------------------------------------------------------------------

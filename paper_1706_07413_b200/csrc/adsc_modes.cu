@@ -5,7 +5,8 @@
 // at x = pi/2, as for the mass, R15),  E_j = Pi_j^2 + Phi_j^2 / omega_j^2  (R24; sum_j E_j -> M in the linear limit).
 // It is a [J x N] . [N x B] contraction whose left factor is never stored: every thread rebuilds the J mode
 // values of its grid points with the three-term Jacobi recurrence, 2F1(-j,3+j;3/2;z) = j!/(3/2)_j P_j^{(1/2,3/2)}(1-2z)
-// and dP_j^{(a,b)}/dy = (j+a+b+1)/2 P_{j-1}^{(a+1,b+1)}.  One CTA per member; off the per-stage path.
+// and dP_j^{(a,b)}/dy = (j+a+b+1)/2 P_{j-1}^{(a+1,b+1)}.  A member is cut into S interleaved slices, one CTA each
+// (k_mode_partial), and the slice partials are summed in a fixed order (k_mode_finish); off the per-stage path.
 #include <cmath>
 
 #include "adsc_internal.cuh"
@@ -24,23 +25,31 @@ struct ModeCoef {
     double iom2[MODES_MAX];      // 1/omega_j^2
 };
 
+// Partial sums of one slice of a member: CTA (b, sl) takes the points i = sl*256 + tid, + S*256, ... (S = gridDim.y
+// slices per member) and leaves sum_i w_i tan^2 x_i Pi_i e_j(x_i) / d'_j and the same for Phi e_j' in
+// part[b][sl][{0,1}][j] (d'_j = d_j j!/(3/2)_j is applied by k_mode_finish).  Per point and mode: the two Jacobi
+// recurrences (6 FP64 instructions) and 4 for the two projections; the weights that do not depend on j are
+// formed once per point.
 __global__ void __launch_bounds__(MODES_THREADS)
-k_mode_energies(Problem pb, Tables tb, const double *__restrict__ gPhi, const double *__restrict__ gPi,
-                const __grid_constant__ ModeCoef mc, int J, double *__restrict__ out)
+k_mode_partial(Problem pb, Tables tb, const double *__restrict__ gPhi, const double *__restrict__ gPi,
+               const __grid_constant__ ModeCoef mc, int J, double *__restrict__ part)
 {
     __shared__ double red[2][MODES_THREADS / 32];
-    const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b = blockIdx.x, sl = blockIdx.y, S = gridDim.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = pb.N;
     const double *Phi = gPhi + (size_t)b * pb.NP, *Pi = gPi + (size_t)b * pb.NP;
     double sp[MODES_MAX], sf[MODES_MAX];
 #pragma unroll
     for (int j = 0; j < MODES_MAX; ++j) { sp[j] = 0.0; sf[j] = 0.0; }
-    for (int i = tid; i < N - 1; i += MODES_THREADS) {        // the integrand is 0 at i = N-1
+    for (int i = sl * MODES_THREADS + tid; i < N - 1; i += S * MODES_THREADS) {        // the integrand is 0 at i = N-1
         double s, c;
         sincospi((double)i / (2.0 * (double)(N - 1)), &s, &c);
-        const double y = c * c - s * s, s2 = 2.0 * s * c, c2 = c * c, c3 = c2 * c;
+        const double y = c * c - s * s, c2 = c * c, c3 = c2 * c;
         const double wt = tb.w[i] * tb.T[i];
-        const double wp = wt * Pi[i], wf = wt * Phi[i];
+        const double wp = (wt * Pi[i]) * c3;                     // Pi e_j = d'_j c^3 P_j
+        const double wf = wt * Phi[i];
+        const double wfa = wf * (-3.0 * c2 * s);                 // Phi e_j' = d'_j (-3 c^2 s P_j - 4 s c^4 dq_j Q_{j-1})
+        const double wfb = wf * (-4.0 * s * c * c3);
         double p0 = 1.0, p1 = mc.p1c[0][0] + mc.p1c[0][1] * (y - 1.0);      // P_{j-1}, P_j of (1/2, 3/2) at j = 1
         double q0 = 0.0, q1 = 1.0;                                          // Q_{j-2}, Q_{j-1} of (3/2, 5/2) at j = 1
 #pragma unroll
@@ -50,21 +59,20 @@ k_mode_energies(Problem pb, Tables tb, const double *__restrict__ gPhi, const do
                 if (j == 0) { Pj = 1.0; Qjm1 = 0.0; }
                 else if (j == 1) { Pj = p1; Qjm1 = 1.0; }
                 else {
-                    const double p2 = (mc.r1[0][j] * y + mc.r2[0][j]) * p1 - mc.r3[0][j] * p0;
+                    const double p2 = fma(fma(mc.r1[0][j], y, mc.r2[0][j]), p1, -mc.r3[0][j] * p0);
                     p0 = p1; p1 = p2; Pj = p2;
                     double q2;                                              // Q_{j-1}: index n = j-1 of family 1
                     if (j == 2) q2 = mc.p1c[1][0] + mc.p1c[1][1] * (y - 1.0);
-                    else q2 = (mc.r1[1][j - 1] * y + mc.r2[1][j - 1]) * q1 - mc.r3[1][j - 1] * q0;
+                    else q2 = fma(fma(mc.r1[1][j - 1], y, mc.r2[1][j - 1]), q1, -mc.r3[1][j - 1] * q0);
                     q0 = q1; q1 = q2; Qjm1 = q2;
                 }
-                const double e = mc.dn[j] * c3 * Pj;
-                const double de = mc.dn[j] * (-3.0 * c2 * s * Pj - 2.0 * s2 * c3 * mc.dq[j] * Qjm1);
-                sp[j] = fma(wp, e, sp[j]);
-                sf[j] = fma(wf, de, sf[j]);
+                sp[j] = fma(wp, Pj, sp[j]);
+                sf[j] = fma(wfa, Pj, fma(wfb * mc.dq[j], Qjm1, sf[j]));
             }
         }
     }
     // CTA reduction, mode by mode (fixed order: deterministic)
+    double *dst = part + ((size_t)b * S + sl) * 2 * J;
 #pragma unroll 1
     for (int j = 0; j < J; ++j) {
         double a = 0.0, f = 0.0;
@@ -81,9 +89,25 @@ k_mode_energies(Problem pb, Tables tb, const double *__restrict__ gPhi, const do
         if (tid == 0) {
             double A = 0.0, F = 0.0;
             for (int w = 0; w < MODES_THREADS / 32; ++w) { A += red[0][w]; F += red[1][w]; }
-            out[(size_t)b * J + j] = A * A + F * F * mc.iom2[j];
+            dst[j] = A; dst[J + j] = F;
         }
     }
+}
+
+// E_j = Pi_j^2 + Phi_j^2 / omega_j^2 from the slice partials, summed in slice order (deterministic).
+__global__ void k_mode_finish(int B, int S, int J, const __grid_constant__ ModeCoef mc, const double *__restrict__ part,
+                              double *__restrict__ out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= B * J) return;
+    const int b = k / J, j = k - b * J;
+    double A = 0.0, F = 0.0;
+    for (int sl = 0; sl < S; ++sl) {
+        const double *src = part + ((size_t)b * S + sl) * 2 * J;
+        A += src[j]; F += src[J + j];
+    }
+    A *= mc.dn[j]; F *= mc.dn[j];
+    out[k] = A * A + F * F * mc.iom2[j];
 }
 
 // coefficients of the Jacobi recurrence 2n(n+a+b)(2n+a+b-2) P_n =
@@ -114,11 +138,32 @@ static void fill_coef(ModeCoef &mc)
     }
 }
 
-cudaError_t launch_mode_energies(adsc_ctx *c, int J, double *d_out)
+// d_out: [B][J]; scratch: at least B * S * 2 * J doubles.  Slices per member: enough CTAs for two waves of the
+// device when the batch alone does not give them, never fewer than 1024 points per CTA.
+int mode_slices(const adsc_ctx *c, int J, size_t scratch_doubles)
+{
+    const int sms = c->dev_sms > 0 ? c->dev_sms : 148;
+    int S = (2 * sms + c->pb.B - 1) / c->pb.B;
+    const int smax_pts = (c->pb.N + 1023) / 1024;
+    if (S > smax_pts) S = smax_pts;
+    const size_t smax_mem = scratch_doubles / ((size_t)c->pb.B * 2 * J);
+    if ((size_t)S > smax_mem) S = (int)smax_mem;
+    if (S > 65535) S = 65535;
+    return S < 1 ? 1 : S;
+}
+
+cudaError_t launch_mode_energies(adsc_ctx *c, int J, double *d_out, double *scratch, size_t scratch_doubles)
 {
     ModeCoef mc;
     fill_coef(mc);
-    k_mode_energies<<<c->pb.B, MODES_THREADS, 0, c->stream>>>(c->pb, c->tb, c->ws.U[0], c->ws.U[1], mc, J, d_out);
+    const int S = mode_slices(c, J, scratch_doubles);
+    k_mode_partial<<<dim3((unsigned)c->pb.B, (unsigned)S), MODES_THREADS, 0, c->stream>>>(c->pb, c->tb, c->ws.U[0], c->ws.U[1],
+                                                                                        mc, J, scratch);
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const int n = c->pb.B * J;
+    k_mode_finish<<<(n + 127) / 128, 128, 0, c->stream>>>(c->pb.B, S, J, mc, scratch, d_out);
     c->launches++;
     return cudaGetLastError();
 }

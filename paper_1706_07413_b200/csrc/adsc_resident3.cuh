@@ -1,4 +1,4 @@
-// adsc_resident3.cu — resident RK4 kernel, third generation ("v3"): one ensemble member per CTA
+// adsc_resident3.cuh — resident RK4 kernel, third generation ("v3"): one ensemble member per CTA
 // (or per cluster of CL CTAs), the whole state on chip across all RK stages and steps.
 //
 // Arithmetic per stage: telescoped delta rule, two synchronisation points per RK
@@ -18,7 +18,12 @@
 //     instructions) and had no register to spare.
 //   * The member-level scan step is a branch-free, fully unrolled, predicated sum of the published warp
 //     totals (two dependent-add chains) instead of a loop of dependent shared-memory loads.
-//   * The cluster size is a template parameter (1, 2, 4, 8).
+//   * The cluster size is a template parameter: any size 1..8 and 16 (the non-portable maximum: 16 x 2048 points
+//     hold the paper's production grid of 2^15 points).
+//   * The member-level scan step leaves the critical path: the exponents of a thread's points are formed WITHOUT
+//     the sum B of everything above the thread, the differences to the reference point do not contain it, and B
+//     enters only the one full exponential per thread, e^{x_ref + (h/2) B}.  B itself is summed by the lanes of a
+//     warp in parallel (one published total per lane, five shuffle steps) while the relative polynomials run.
 //
 // Per RK stage (equations PAPER.md:43-53 eqs (2)-(6); boundary conditions PAPER.md:59-75):
 //   phase 1  (after sync S: neighbours' Phi, Pi edges + warp totals of f)  delta, E = e^{-delta},
@@ -26,35 +31,13 @@
 //   phase 2  Kreiss-Oliger Q Phi, Q Pi and interior D4 (before the wait), edge D4, RK combine for
 //            Phi, Pi, collapse test (stage 4), f of the NEW state, thread/warp scan,
 //            publish Phi, Pi edges + warp totals                                             -> sync S
+#pragma once
 #include "adsc_internal.cuh"
 #include "adsc_resident.cuh"
 #include "adsc_exp.cuh"
 #include "adsc_ptx.cuh"
 
 namespace adsc {
-
-template <int P, int THREADS, bool ACC_REG, int CL>
-struct Res3Layout {
-    static constexpr int SEG = P * THREADS;
-    static constexpr int LD = THREADS + 2;          // halo column on each side
-    static constexpr int NW = THREADS / 32;
-    static constexpr int NG = NW * CL;              // warps per member
-    static constexpr int RX = (P < 6) ? P : 6;      // rows of the state exchange buffers
-    static constexpr int o_xPhi = 0;
-    static constexpr int o_xPi = o_xPhi + RX * LD;
-    static constexpr int o_xH = o_xPi + RX * LD;
-    static constexpr int o_xF = o_xH + 4 * LD;
-    static constexpr int o_tSC = o_xF + 4 * LD;      // -2 sin x cos x, [P][LD] with halo columns
-    static constexpr int o_tT = o_tSC + P * LD;      // tan^2 x
-    static constexpr int o_tC = o_tT + P * THREADS;  // cot^2 x / (12 h)
-    static constexpr int o_un = o_tC + P * THREADS;
-    static constexpr int o_acc = o_un + 3 * P * THREADS;
-    static constexpr int o_wt = o_acc + (ACC_REG ? 0 : 3 * P * THREADS);   // [2][NG] {total, flag}
-    static constexpr int o_mbar = o_wt + 2 * NG * 2;                       // mbS[0], mbS[1], mbF, pad
-    static constexpr int n_doubles = o_mbar + 4;
-    static constexpr size_t bytes = (size_t)n_doubles * sizeof(double);
-    static_assert(o_wt % 2 == 0, "warp-total slots must be 16-byte aligned");
-};
 
 // FIXED: the paper's second workload (Table II), A = 1 and delta = 0 held fixed: no f', no scan,
 // no exponential, eq (4) not evolved, no collapse test -- the same stencils, exchanges and RK combine.
@@ -73,6 +56,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
 #ifndef ADSC_R3_NFILL
 #define ADSC_R3_NFILL 3
 #endif
+#ifndef ADSC_R3_LANESUM_MIN_NG
+#define ADSC_R3_LANESUM_MIN_NG 32
+#endif
+    constexpr bool LANESUM = NG >= ADSC_R3_LANESUM_MIN_NG;              // member-level sum by the lanes of the warp
     constexpr bool EARLY = ADSC_R3_EARLY && (P >= 6);                   // interior right-hand sides before the sync-F wait
     constexpr int NFILL = (P < ADSC_R3_NFILL) ? P : ADSC_R3_NFILL;      // Kreiss-Oliger points computed inside the shuffle chain
     extern __shared__ __align__(16) double smem[];
@@ -281,9 +268,21 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 for (int p = 0; p < P; ++p) E[p] = 1.0;                   // delta = 0 held fixed
             } else {
                 const double scm = tSC[(P - 1) * LD + col - 1], scp = tSC[0 * LD + col + 1];
-                // a2, member level: all f' above this thread's points (predicates are warp- / CTA-uniform)
-                double B0 = excl, B1 = 0.0;
-                {
+                // a2, member level: the sum B of all f' above this thread's points.  It enters only the reference
+                // exponential of the thread (see exp3_near), so the sum runs beside the arithmetic below.
+                double B;
+                if constexpr (LANESUM) {
+                    double v = 0.0;
+#pragma unroll
+                    for (int k = 0; k < (NG + 31) / 32; ++k) {
+                        const int idx = lane + 32 * k;
+                        if (idx < NG) { const double t = wts[idx].x; v += (idx > gw) ? t : 0.0; }
+                    }
+#pragma unroll
+                    for (int d = 16; d >= 1; d >>= 1) v += __shfl_xor_sync(FULL, v, d);
+                    B = excl + v;
+                } else {                    // few warps: predicated serial sum (predicates are warp- / CTA-uniform)
+                    double B0 = excl, B1 = 0.0;
                     const double2 *wl = wts + rank * NW;
 #pragma unroll
                     for (int w = 1; w < NW; ++w) {
@@ -298,9 +297,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                             }
                         }
                     }
+                    B = B0 + B1;
                 }
-                const double B = B0 + B1;
-                // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f
+                // a1/a2: -delta_p = (h/2)(s_{p+2} + B) + (h/48)(25 f'_{p+1} + 12 f'_p - f'_{p-1}),  f' = -2 f;
+                // nd holds it without the (h/2) B term
                 double nd[P];
                 {
                     const double fm = scm * fma(hlP[2], hlP[2], hlQ[2] * hlQ[2]);     // f'_{-1}
@@ -314,10 +314,10 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                         double loc = K.c25 * f_hi;
                         loc = fma(K.c12, fo[p], loc);
                         loc = fma(-K.c1, f_lo, loc);
-                        nd[p] = fma(K.hh, s2 + B, loc);
+                        nd[p] = fma(K.hh, s2, loc);
                     }
                 }
-                exp3_near<P>(nd, E);
+                exp3_near<P, false, true>(nd, E, 1.0, nullptr, K.hh * B);
             }
             // a3 fluxes
             double H[P], F[P], kAv[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;
@@ -467,7 +467,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                 if constexpr (!FIXED) {
                     const int2 *fl = reinterpret_cast<const int2 *>(wt + jb * NG);
 #pragma unroll
-                    for (int w = 0; w < NG; ++w) any |= fl[2 * w + 1].y;  // high word of the flag (0.0 or 1.0)
+                    for (int k = 0; k < (NG + 31) / 32; ++k) {
+                        const int idx = lane + 32 * k;
+                        if (idx < NG) any |= fl[2 * idx + 1].y;           // high word of the flag (0.0 or 1.0)
+                    }
+                    any = __any_sync(FULL, any != 0);
                 }
                 n_done = n + 1;
                 if (any && (prm.check_last || n + 1 < prm.nsteps)) collapsed = 1;
@@ -496,46 +500,5 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
     // no CTA may exit while a peer can still store into its shared memory
     if (MULTI) asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-
-// ------------------------------------------------------------------ configuration table
-#define ADSC_RES3_FN(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false, 4>
-#define ADSC_RES3_FNF(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, true, 4>
-#define ADSC_RES3_FN3(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false, 3>
-#define ADSC_RES3_FN2(P_, T_, ACC_, CL_) (const void *)k_resident3<P_, T_, ACC_, CL_, false, 2>
-// fn: dynamical A, delta, RK4; fnf: fixed background; fn3, fn2: Runge-Kutta orders 3 and 2 (R25);
-// nullptr where not compiled (tuning variants)
-#define ADSC_RES3_CFG_ALL(P_, T_, ACC_)                                                               \
-    { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 8>::bytes, false,       \
-      { ADSC_RES3_FN(P_, T_, ACC_, 1), ADSC_RES3_FN(P_, T_, ACC_, 2), ADSC_RES3_FN(P_, T_, ACC_, 4),    \
-        ADSC_RES3_FN(P_, T_, ACC_, 8) },                                                              \
-      { ADSC_RES3_FNF(P_, T_, ACC_, 1), ADSC_RES3_FNF(P_, T_, ACC_, 2), ADSC_RES3_FNF(P_, T_, ACC_, 4), \
-        ADSC_RES3_FNF(P_, T_, ACC_, 8) },                                                             \
-      { ADSC_RES3_FN3(P_, T_, ACC_, 1), ADSC_RES3_FN3(P_, T_, ACC_, 2), ADSC_RES3_FN3(P_, T_, ACC_, 4), \
-        ADSC_RES3_FN3(P_, T_, ACC_, 8) },                                                             \
-      { ADSC_RES3_FN2(P_, T_, ACC_, 1), ADSC_RES3_FN2(P_, T_, ACC_, 2), ADSC_RES3_FN2(P_, T_, ACC_, 4), \
-        ADSC_RES3_FN2(P_, T_, ACC_, 8) } }
-#define ADSC_RES3_CFG_ONE(P_, T_, ACC_)                                                               \
-    { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 1>::bytes, false,       \
-      { ADSC_RES3_FN(P_, T_, ACC_, 1), nullptr, nullptr, nullptr },                                   \
-      { ADSC_RES3_FNF(P_, T_, ACC_, 1), nullptr, nullptr, nullptr },                                  \
-      { ADSC_RES3_FN3(P_, T_, ACC_, 1), nullptr, nullptr, nullptr },                                  \
-      { ADSC_RES3_FN2(P_, T_, ACC_, 1), nullptr, nullptr, nullptr } }
-#define ADSC_RES3_CFG_TUNE(P_, T_, ACC_)                                                              \
-    { "v3P" #P_ "xT" #T_ #ACC_, P_, T_, P_ * T_, ACC_, Res3Layout<P_, T_, ACC_, 8>::bytes, false,       \
-      { ADSC_RES3_FN(P_, T_, ACC_, 1), ADSC_RES3_FN(P_, T_, ACC_, 2), ADSC_RES3_FN(P_, T_, ACC_, 4),    \
-        ADSC_RES3_FN(P_, T_, ACC_, 8) },                                                              \
-      { nullptr, nullptr, nullptr, nullptr }, { nullptr, nullptr, nullptr, nullptr },               \
-      { nullptr, nullptr, nullptr, nullptr } }
-
-const ResConfig g_cfgs3[] = {
-    ADSC_RES3_CFG_ALL(8, 256, true),    // SEG 2048, accumulators in registers: N-1 = 2048, 4096, 8192, 16384
-    ADSC_RES3_CFG_ONE(8, 128, false),   // SEG 1024
-    ADSC_RES3_CFG_ONE(4, 128, false),   // SEG 512
-    ADSC_RES3_CFG_ONE(4, 64, false),    // SEG 256
-    ADSC_RES3_CFG_ONE(4, 32, false),    // SEG 128
-    ADSC_RES3_CFG_TUNE(8, 128, true),   // SEG 1024, two CTAs per SM (tuning)
-    ADSC_RES3_CFG_TUNE(4, 512, true),   // SEG 2048, 16 warps (tuning)
-};
-const int n_cfgs3 = sizeof(g_cfgs3) / sizeof(g_cfgs3[0]);
 
 }  // namespace adsc

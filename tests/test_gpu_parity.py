@@ -553,7 +553,8 @@ def test_collapse_with_A_resolve_period(env, path, K_A):
 SANITIZER_CASES = [
     # (N, B, path, kw): one launch of every stage-kernel family and cluster size, 3 steps
     (17, 2, 3, {}), (33, 2, 1, {}), (33, 2, 3, {}), (129, 2, 2, {}), (1025, 2, 2, {}), (1025, 2, 1, {}),
-    (2049, 2, 2, {}), (3073, 2, 0, {}), (4097, 2, 2, {}), (8193, 2, 2, {}), (16385, 1, 2, {}),
+    (2049, 2, 2, {}), (3073, 2, 0, {}), (4097, 2, 2, {}), (6145, 2, 2, {}), (8193, 2, 2, {}), (16385, 1, 2, {}),
+    (32769, 1, 2, {}),
     (20481, 3, 1, {}), (4097, 2, 2, dict(rk_order=3)), (2049, 2, 2, dict(fixed_background=True)),
     (20481, 2, 1, dict(fixed_background=True)),
 ]
@@ -573,3 +574,85 @@ def test_short_runs_every_kernel_family(env, N, B, path, kw):
     else:
         _compare(f, ev)
     assert (d["steps_done"] == 3).all()
+
+
+@pytest.mark.parametrize("N,B,nsteps,kw", [
+    (6145, 3, 1000, {}),                      # cluster of 3
+    (10241, 2, 400, {}),                      # 5
+    (12289, 2, 300, dict(rk_order=3)),        # 6
+    (14337, 2, 300, {}),                      # 7
+    (16385, 2, 300, {}),                      # 8
+    (32769, 9, 100, {}),                      # 16 (non-portable cluster size): more members than co-resident clusters
+    (32769, 2, 200, dict(rk_order=3)),        # the paper's production shape: 2^15 points, RK3
+    (32769, 2, 100, dict(fixed_background=True)),
+])
+def test_resident_every_cluster_size(env, N, B, nsteps, kw):
+    """Resident kernel on clusters of 3, 5, 6, 7, 8 and 16 CTAs of 2048 points (1, 2 and 4 are the config shapes)."""
+    name = "paper32k" if (N == 32769 and kw.get("rk_order") == 3) else "cfg2"
+    Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
+    ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=2, **kw)
+    assert ens.path == (2, (N - 1) // 2048)
+    okw = dict(fixed_background=True) if kw.get("fixed_background") else {}
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 8), rk_order=kw.get("rk_order", 4), **okw).step(nsteps)
+    if kw.get("fixed_background"):
+        assert np.max(np.abs(f["Phi"] - ev.Phi)) <= TOL and np.max(np.abs(f["Pi"] - ev.Pi)) <= TOL
+    else:
+        _compare(f, ev)
+        _bc_invariants(f)
+    assert (d["steps_done"] == nsteps).all() and (d["collapsed"] == 0).all()
+
+
+@pytest.mark.parametrize("N", [6145, 32769])
+def test_collapse_on_wide_clusters(env, N):
+    """Collapse flags raised in the first and in an outer CTA of a cluster of 3 / 16 reach every CTA: the threshold
+    is put between the oracle's min A after 40 and after 80 steps of one member (its min A falls by 1e-6..1e-4 in
+    between: far above the 1e-13 agreement of the two codes), so that this member collapses in mid-run; flags,
+    collapse times, step counts and the states (frozen or not) as the oracle's."""
+    B, n1, n2, ntot = 4, 40, 80, 160
+    x = env["inputs"].grid(N)
+    Pi = env["inputs"].gaussian_Pi(N, [100.0, 1.0, 1.0, 2.0], np.full(B, 1.0 / 16))
+    Pi[1] += 6.0 * np.exp(-((x - 1.0) / 0.05) ** 2)             # member 1: min A at x ~ 1, in an outer CTA
+    Pi[:, -1] = 0.0
+    Phi = np.tile(2.0 * np.sin(2 * x) * np.cos(x) ** 2, (B, 1))
+    Phi[:, 0] = 0.0; Phi[:, -1] = 0.0
+    pre = env["oracle"].Evolution(Phi, Pi, thr=0.0, nthreads=4).step(n1)
+    m1 = pre.A.min(axis=1)
+    pre.step(n2 - n1)
+    m2 = pre.A.min(axis=1)
+    assert (pre.A.argmin(axis=1)[1] // 2048) >= 1
+    for who in (0, 1):
+        assert m2[who] < m1[who] - 1e-8
+        thr = 0.5 * (m1[who] + m2[who])
+        ev = env["oracle"].Evolution(Phi, Pi, thr=thr, nthreads=4).step(ntot)
+        od = ev.diagnostics()
+        assert od["collapsed"][who] == 1 and n1 < od["steps_done"][who] <= n2 and (od["collapsed"] == 0).any()
+        ens, f, d = _gpu_run(env, Phi, Pi, ntot, path=2, threshold=thr)
+        assert ens.path == (2, (N - 1) // 2048)
+        assert (d["collapsed"] == od["collapsed"]).all() and (d["steps_done"] == od["steps_done"]).all()
+        for b in range(B):
+            if od["collapsed"][b]:
+                assert abs(d["t_collapse"][b] - od["t_collapse"][b]) <= ev.dt * 1e-9
+            for k, ref in (("Phi", ev.Phi), ("Pi", ev.Pi), ("A", ev.A)):
+                assert np.max(np.abs(f[k][b] - ref[b])) <= TOL, (b, k)
+
+
+@pytest.mark.parametrize("N,B,path", [(2049, 300, 2), (4097, 150, 2), (8193, 70, 2), (32769, 12, 2), (6145, 60, 2),
+                                      (20481, 40, 1), (2 ** 18 + 1, 2, 1), (32769, 40, 1)])
+def test_bitwise_reproducible(env, N, B, path):
+    """Two runs of the same launch give bit-identical fields (more members than one wave of CTAs, so the schedule of
+    CTAs differs between the runs).  compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md); a race in
+    the mbarrier / st.async / mailbox protocols would show here as a run-to-run difference -- this is how the
+    copy-engine-versus-load-queue race of the table ring was found."""
+    torch = env["torch"]
+    Phi, Pi, _ = env["inputs"].make("cfg2", B=B, N=N)
+    Pi = Pi * 3.0
+    outs = []
+    for rep in range(3):
+        ens, f, d = _gpu_run(env, Phi, Pi, 24, path=path)
+        assert ens.path[0] == path
+        outs.append(f)
+        if rep == 1:                                   # perturb the co-scheduling: something else is running beside
+            torch.empty(64 << 20, device="cuda").normal_()
+    for o in outs[1:]:
+        for k in ("Phi", "Pi", "A", "delta"):
+            assert np.array_equal(o[k], outs[0][k]), k
