@@ -57,6 +57,9 @@ def parse():
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "paper32k"])
     ap.add_argument("--rk4-per-step", type=int, default=0, help="RK4 steps per bench step (0 = workload default)")
     ap.add_argument("--batch", type=int, default=0, help="override the ensemble size (0 = workload default)")
+    ap.add_argument("--grid-points", type=int, default=0, metavar="N",
+                    help="override the grid size N of the workload's data family (diagnosis only: the line then no "
+                         "longer describes a BASELINE.json config; config.N says what ran)")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 persistent streaming, 2 resident, 3 generic streaming")
     ap.add_argument("--fixed-background", action="store_true",
                     help="time the fixed-background variant (A = 1, delta = 0 held fixed; PAPER.md:177 Table II)")
@@ -155,7 +158,7 @@ def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False, rk_order=4, threads
     Bfull = inputs.CONFIGS[name]["B"]
     B = min(Bfull, 2 * thr) if threads is None else threads
     thr = min(thr, B)
-    Phi, Pi, _ = inputs.make(name, B=B)
+    Phi, Pi, _ = inputs.make(name, B=B, N=N)
     ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=fixed, rk_order=rk_order)
     t = time.perf_counter(); ev.step(2); cal = (time.perf_counter() - t) / 2
     n = max(2, int(seconds / max(cal, 1e-9)))
@@ -236,14 +239,14 @@ def main():
 
     name = args.workload
     cfg = inputs.CONFIGS[name]
-    N = cfg["N"]
+    N = args.grid_points or cfg["N"]
     B = args.batch or cfg["B"]              # members PER GPU (weak scaling: members are independent)
     rk4 = args.rk4_per_step or RK4_PER_STEP[name]
     K, W = args.steps, max(args.warmup, 0)
 
     # Rank r evolves members [r*B, (r+1)*B) of the (tiled) seeded ensemble: no exchange step.
     lo, hi = shard.member_range(rank, world, B * world)
-    Phi_all, Pi_all, _ = inputs.make(name, B=hi, lo=lo)       # this rank's members only
+    Phi_all, Pi_all, _ = inputs.make(name, B=hi, lo=lo, N=N)  # this rank's members only
     if args.masked_fraction > 0.0:
         bidx = np.arange(lo, hi)
         forced = np.floor((bidx + 1) * args.masked_fraction) > np.floor(bidx * args.masked_fraction)

@@ -56,6 +56,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
 #ifndef ADSC_R3_NFILL
 #define ADSC_R3_NFILL 3
 #endif
+    // Scope of the acquire in the mbarrier waits that guard data written by peer CTAs: cluster (the formally required
+    // one; ptxas adds an L1 invalidate, CCTL.IVALL, behind such a wait).  Measured with CTA scope instead (the data
+    // lives in shared memory, which no cache holds): no difference (cfg2 0.621 -> 0.623), so the formal scope stays.
 #ifndef ADSC_R3_LANESUM_MIN_NG
 #define ADSC_R3_LANESUM_MIN_NG 32
 #endif
