@@ -84,7 +84,7 @@ def parse():
 
 
 # RK steps per bench step: >= 100 ms per adsc_step call, so that --steps 20 times >= 2 s of GPU work
-RK4_PER_STEP = {"cfg1": 20000, "cfg2": 1200, "cfg3": 150, "cfg4": 1500, "cfg5": 200, "paper32k": 1000}
+RK4_PER_STEP = {"cfg1": 25000, "cfg2": 1200, "cfg3": 150, "cfg4": 1500, "cfg5": 200, "paper32k": 2000}
 WORKLOAD_DESC = {
     "cfg1": "configs[0]: 1 member, N=1025, Gaussian Pi sigma=1/16 eps=1",
     "cfg2": "configs[1]: amplitude ensemble, 1024 members, N=4097, Gaussian Pi sigma=1/16 eps~U[0.5,5]",
@@ -383,6 +383,8 @@ def main():
         # [NS]/SURVEY.md 8(d) streaming roofline: bytes per point per step with one fused pass per stage:
         # first and last stage 72 B, every middle stage 120 B
         bytes_step = 72.0 * 2 + 120.0 * (NS - 2)
+        if args.fixed_background:
+            bytes_step *= 2.0 / 3.0                       # two evolved fields instead of three
         ach = per_gpu_rate * bytes_step / 1e9
         kern_bytes = (STREAM_BYTES_STAGE_FIRST + STREAM_BYTES_STAGE_LAST + STREAM_BYTES_STAGE_MID * (NS - 2)
                       + STREAM_BYTES_TABLES * NS)

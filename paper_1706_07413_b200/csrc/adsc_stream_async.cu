@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     // token of the mbarrier arrive (adsc_ptx.cuh).  Without this a queued load could read the NEXT slice's table.
     auto ring_next = [&](int t, int j, unsigned dep) {
         if (reload) {
-            dep = __reduce_or_sync(FULL, dep);
+            // (lane 0's words are enough: a load is one warp instruction, its registers are released together)
             ring_issue(t, SA_NW * (j > 0 ? j - 1 : n_my - 1) + warp, dep);
             phs ^= 1u << t;
         }
@@ -432,9 +432,12 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                 double Cst = 1.0;                                         // C, once this stage's gather is done
                 const uint32_t cpar = (phs >> 4) & 1u;
                 phs ^= 16u;
-                for (int j = NT - 1; j >= 0; --j) {
+                bool tile1 = true, tile2 = false;                         // the stage's first / second tile (no reload of NT)
+                for (int j = (NQ + SA_NW - 1) / SA_NW - 1; j >= 0; --j) {
                     // the first tile of the stage works with delta_local and takes C in at its end
-                    const bool defer = !FIXED && (j == NT - 1);
+                    const bool defer = !FIXED && tile1;
+                    const bool after_defer = tile2;
+                    tile2 = tile1; tile1 = false;
                     if (j >= n_my) {                                      // ragged top tile: nothing to do for this warp
                         if (defer) {
                             if (warp == SA_WH) gather(par);
@@ -683,7 +686,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     if (lane == 31) {
                         const double2 *src = (q + 1 < NQ) ? flo2 + 2 * (q + 1) : ftop2;
                         const double2 x = src[0], y = src[1];
-                        const double m = (!FIXED && !defer && q + 1 == SA_NW * (NT - 1)) ? Cst : 1.0;
+                        const double m = (!FIXED && after_defer && warp == SA_NW - 1) ? Cst : 1.0;     // (q + 1 is the first slice of the first tile)
                         Hp0 = x.x * m; Hp1 = x.y * m; Fp0 = y.x * m; Fp1 = y.y * m;
                     }
                     if (first) { Hm2 = H[2]; Hm1 = H[1]; Fm2 = -F[2]; Fm1 = -F[1]; }      // x=0: H even, F odd
