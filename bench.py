@@ -171,6 +171,33 @@ def oracle_rate(name, N, seconds, rk4_cap=None, fixed=False, rk_order=4, threads
                        f"gcc -O2 -ffp-contract=off, OpenMP over members"), el, n, B
 
 
+def fast_build_rate(name, N, seconds, fixed, rk_order):
+    """The oracle's source compiled for throughput (gcc -O3 -march=native -ffp-contract=fast; oracle.build_fast) on the
+    same sample and cores, checked against the oracle over 20 steps first.  Reported beside the oracle's rate: the
+    oracle is the unoptimised checker, this is the same program as a compiler makes it fast."""
+    import oracle
+    from paper_1706_07413_b200 import inputs
+    try:
+        thr = min(os.cpu_count() or 1, oracle.max_threads())
+        B = min(inputs.CONFIGS[name]["B"], thr)
+        thr = min(thr, B)
+        Phi, Pi, _ = inputs.make(name, B=B, N=N)
+        ref = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=fixed, rk_order=rk_order).step(20)
+        oracle.use_build("fast")
+        ev = oracle.Evolution(Phi, Pi, nthreads=thr, fixed_background=fixed, rk_order=rk_order).step(20)
+        diff = float(max(np.max(np.abs(ev.Phi - ref.Phi)), np.max(np.abs(ev.Pi - ref.Pi)), np.max(np.abs(ev.A - ref.A))))
+        t = time.perf_counter(); ev.step(2); cal = (time.perf_counter() - t) / 2
+        n = max(2, int(seconds / max(cal, 1e-9)))
+        t = time.perf_counter(); ev.step(n); el = time.perf_counter() - t
+        return {"value": B * N * n / el, "unit": UNIT, "cores": thr, "flags": " ".join(oracle.FAST_FLAGS),
+                "max_abs_diff_vs_oracle_20_steps": diff,
+                "sample": f"{B} members of {name} (N={N}) x {n} steps, {el:.1f} s"}
+    except Exception as e:                                  # (a missing -march=native target etc.: no fast figure)
+        return {"value": None, "error": str(e)[:200]}
+    finally:
+        oracle.use_build("oracle")
+
+
 # ----------------------------------------------------------------------------- reference arm
 def run_reference(args):
     """`--impl reference`: the oracle as it stands on the host cores, same config/metric/unit.
@@ -413,6 +440,7 @@ def main():
         one, _, _, _ = oracle_rate(name, N, min(5.0, args.cpu_seconds), fixed=args.fixed_background,
                                    rk_order=args.rk_order, threads=1)
         cpu["one_core"] = {"value": one["value"], "unit": UNIT, "cores": 1, "sample": one["sample"]}
+        cpu["fast_build"] = fast_build_rate(name, N, min(5.0, args.cpu_seconds), args.fixed_background, args.rk_order)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,

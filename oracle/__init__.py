@@ -29,13 +29,49 @@ def build(force: bool = False) -> str:
     return _SO
 
 
+
+
+def _cpu_tag() -> str:
+    """-march=native code only runs on the CPU model it was built on: one library per model."""
+    import hashlib
+    try:
+        with open("/proc/cpuinfo") as f:
+            flags = next((l for l in f if l.startswith("flags")), "")
+    except OSError:
+        flags = ""
+    return hashlib.sha1(flags.encode()).hexdigest()[:10]
+
+
+_SO_FAST = os.path.join(_HERE, f"libadsc_oracle_fast_{_cpu_tag()}.so")
+FAST_FLAGS = ["-O3", "-march=native", "-ffp-contract=fast"]
+
+
+def build_fast(force: bool = False) -> str:
+    """The SAME source with throughput flags (gcc -O3 -march=native, contraction allowed), as a second library.
+    It is not the oracle: bench.py times it beside the oracle so that the CPU baseline is not only the unoptimised
+    checker, and checks it against the oracle before quoting it."""
+    if force or not os.path.exists(_SO_FAST) or os.path.getmtime(_SO_FAST) < os.path.getmtime(_SRC):
+        tmp = _SO_FAST + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-std=c11", *FAST_FLAGS, "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _SO_FAST)
+    return _SO_FAST
+
+
 _lib = None
+_libs = {}
+
+
+def use_build(which: str = "oracle"):
+    """Select the library the wrappers below call: "oracle" (default; the checker) or "fast" (build_fast)."""
+    global _lib
+    if which not in _libs:
+        _libs[which] = C.CDLL(build() if which == "oracle" else build_fast())
+    _lib = _libs[which]
 
 
 def lib():
-    global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
+        use_build("oracle")
     return _lib
 
 

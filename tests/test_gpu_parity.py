@@ -656,3 +656,18 @@ def test_bitwise_reproducible(env, N, B, path):
     for o in outs[1:]:
         for k in ("Phi", "Pi", "A", "delta"):
             assert np.array_equal(o[k], outs[0][k]), k
+
+
+def test_roofline_probes_are_plausible(env):
+    """adsc_probe (the denominators bench.py reports as measured): FP64 FMA rate below the derived peak of the device
+    and above half of it; conflict-free 128-bit shared-memory loads between 64 and 128 B per clock and SM."""
+    torch, binding = env["torch"], env["binding"]
+    prop = torch.cuda.get_device_properties(0)
+    sms = prop.multi_processor_count
+    fp64 = binding.adsc_probe(binding.ADSC_PROBE_FP64_FMA, 20.0)
+    lds = binding.adsc_probe(binding.ADSC_PROBE_SHARED_LOAD, 20.0)
+    peak = sms * 64 * 2 * 1.965e9                       # 64 DFMA lanes per SM at the B200's boost clock
+    assert 0.5 * peak < fp64 <= 1.02 * peak, (fp64, peak)
+    assert 64 * sms * 1.0e9 < lds < 128 * sms * 2.1e9, lds
+    lib = binding.load_library()
+    assert lib.adsc_probe(7, 10.0, None) == binding.ADSC_EINVAL
