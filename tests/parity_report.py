@@ -16,6 +16,9 @@ sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 CASES = [  # name, B, steps, rk_order
     ("cfg1", 1, 1000, 4), ("cfg2", 8, 1000, 4), ("cfg3", 8, 1000, 4), ("cfg4", 1, 20, 4), ("cfg5", 8, 1000, 4),
     ("paper32k", 2, 200, 3),
+    # the configs' own run lengths (BASELINE.json: cfg1 to t = 10, cfg3 20000 steps, cfg4 1000 steps): information only,
+    # the [NS] tolerance is stated for 1000 steps
+    ("cfg1", 1, 26076, 4), ("cfg3", 4, 20000, 4), ("cfg4", 1, 1000, 4),
 ]
 
 
