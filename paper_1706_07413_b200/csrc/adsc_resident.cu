@@ -13,18 +13,18 @@ static const void *fn_big(int cl, int kind)
     if (const void *f = res3_big_b(cl, kind)) return f;
     return res3_big_c(cl, kind);
 }
-static const void *fn_1024(int cl, int kind) { return cl == 1 ? res3_small(1024, kind) : nullptr; }
-static const void *fn_512(int cl, int kind) { return cl == 1 ? res3_small(512, kind) : nullptr; }
-static const void *fn_256(int cl, int kind) { return cl == 1 ? res3_small(256, kind) : nullptr; }
-static const void *fn_128(int cl, int kind) { return cl == 1 ? res3_small(128, kind) : nullptr; }
+static const void *fn_1024(int cl, int kind) { return cl == 1 ? res3_small(1024, kind) : res3_small_odd(1024, cl, kind); }
+static const void *fn_512(int cl, int kind) { return cl == 1 ? res3_small(512, kind) : res3_small_odd(512, cl, kind); }
+static const void *fn_256(int cl, int kind) { return cl == 1 ? res3_small(256, kind) : res3_small_odd(256, cl, kind); }
+static const void *fn_128(int cl, int kind) { return cl == 1 ? res3_small(128, kind) : res3_small_odd(128, cl, kind); }
 
 // widest segment first
 static const ResConfig g_cfgs[] = {
     { "P8xT256", 8, 256, 2048, true, Res3Layout<8, 256, true, RES_MAX_CLUSTER>::bytes, fn_big },   // N-1 = cl x 2048, cl in 1..8, 16
-    { "P8xT128", 8, 128, 1024, false, Res3Layout<8, 128, false, 1>::bytes, fn_1024 },
-    { "P4xT128", 4, 128, 512, false, Res3Layout<4, 128, false, 1>::bytes, fn_512 },
-    { "P4xT64", 4, 64, 256, false, Res3Layout<4, 64, false, 1>::bytes, fn_256 },
-    { "P4xT32", 4, 32, 128, false, Res3Layout<4, 32, false, 1>::bytes, fn_128 },
+    { "P8xT128", 8, 128, 1024, false, Res3Layout<8, 128, false, 7>::bytes, fn_1024 },                // cl = 1, 3, 5, 7
+    { "P4xT128", 4, 128, 512, false, Res3Layout<4, 128, false, 7>::bytes, fn_512 },
+    { "P4xT64", 4, 64, 256, false, Res3Layout<4, 64, false, 7>::bytes, fn_256 },
+    { "P4xT32", 4, 32, 128, false, Res3Layout<4, 32, false, 7>::bytes, fn_128 },
 };
 constexpr int n_cfgs = sizeof(g_cfgs) / sizeof(g_cfgs[0]);
 

@@ -553,7 +553,7 @@ def test_collapse_with_A_resolve_period(env, path, K_A):
 SANITIZER_CASES = [
     # (N, B, path, kw): one launch of every stage-kernel family and cluster size, 3 steps
     (17, 2, 3, {}), (33, 2, 1, {}), (33, 2, 3, {}), (129, 2, 2, {}), (1025, 2, 2, {}), (1025, 2, 1, {}),
-    (2049, 2, 2, {}), (3073, 2, 0, {}), (4097, 2, 2, {}), (6145, 2, 2, {}), (8193, 2, 2, {}), (16385, 1, 2, {}),
+    (2049, 2, 2, {}), (3073, 2, 2, {}), (641, 2, 2, {}), (4097, 2, 2, {}), (6145, 2, 2, {}), (8193, 2, 2, {}), (16385, 1, 2, {}),
     (32769, 1, 2, {}),
     (20481, 3, 1, {}), (4097, 2, 2, dict(rk_order=3)), (2049, 2, 2, dict(fixed_background=True)),
     (20481, 2, 1, dict(fixed_background=True)),
@@ -576,7 +576,23 @@ def test_short_runs_every_kernel_family(env, N, B, path, kw):
     assert (d["steps_done"] == 3).all()
 
 
+def _resident_cluster(N):
+    """CTAs per member the resident path is expected to choose (widest segment first; adsc_resident.cu)."""
+    for seg in (2048, 1024, 512, 256, 128):
+        if (N - 1) % seg == 0:
+            cl = (N - 1) // seg
+            if (seg == 2048 and (1 <= cl <= 8 or cl == 16)) or (seg < 2048 and cl in (1, 3, 5, 7)):
+                return cl
+    return None
+
+
 @pytest.mark.parametrize("N,B,nsteps,kw", [
+    (3073, 3, 1000, {}),                      # 3 x 1024 points
+    (5121, 2, 300, dict(fixed_background=True)),   # 5 x 1024
+    (7169, 2, 300, {}),                       # 7 x 1024
+    (1537, 3, 500, dict(rk_order=3)),         # 3 x 512
+    (1281, 2, 400, {}),                       # 5 x 256
+    (897, 3, 400, {}),                        # 7 x 128
     (6145, 3, 1000, {}),                      # cluster of 3
     (10241, 2, 400, {}),                      # 5
     (12289, 2, 300, dict(rk_order=3)),        # 6
@@ -587,11 +603,12 @@ def test_short_runs_every_kernel_family(env, N, B, path, kw):
     (32769, 2, 100, dict(fixed_background=True)),
 ])
 def test_resident_every_cluster_size(env, N, B, nsteps, kw):
-    """Resident kernel on clusters of 3, 5, 6, 7, 8 and 16 CTAs of 2048 points (1, 2 and 4 are the config shapes)."""
+    """Resident kernel on clusters of 3, 5, 6, 7, 8 and 16 CTAs of 2048 points (1, 2 and 4 are the config shapes) and on
+    clusters of 3, 5, 7 CTAs of the short segments."""
     name = "paper32k" if (N == 32769 and kw.get("rk_order") == 3) else "cfg2"
     Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
     ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=2, **kw)
-    assert ens.path == (2, (N - 1) // 2048)
+    assert ens.path == (2, _resident_cluster(N))
     okw = dict(fixed_background=True) if kw.get("fixed_background") else {}
     ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 8), rk_order=kw.get("rk_order", 4), **okw).step(nsteps)
     if kw.get("fixed_background"):
