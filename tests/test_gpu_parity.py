@@ -688,3 +688,28 @@ def test_roofline_probes_are_plausible(env):
     assert 64 * sms * 1.0e9 < lds < 128 * sms * 2.1e9, lds
     lib = binding.load_library()
     assert lib.adsc_probe(7, 10.0, None) == binding.ADSC_EINVAL
+
+
+def test_maximum_sizes(env):
+    """The largest batch adsc_create accepts (65535 members, here of N = 129) and the longest member the persistent
+    streaming kernel holds on this device (148 chunks of 7168 points), a few steps each against the oracle."""
+    torch, binding = env["torch"], env["binding"]
+    B, N = 65535, 129
+    Phi, Pi, _ = env["inputs"].make("cfg5", B=B, N=N)
+    ens, f, d = _gpu_run(env, Phi, Pi, 20, path=2)
+    assert ens.path == (2, 1)
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=16).step(20)
+    _compare(f, ev)
+    assert (d["steps_done"] == 20).all()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    N = sms * 7168 + 1
+    Phi, Pi, _ = env["inputs"].make("cfg4", N=N)
+    ens, f, d = _gpu_run(env, Phi, Pi, 3, path=1)
+    assert ens.path == (1, sms)
+    ev = env["oracle"].Evolution(Phi, Pi).step(3)
+    _compare(f, ev)
+    _bc_invariants(f)
+    with pytest.raises(binding.AdscError):
+        binding.Ensemble(N + 8, 1, path=2)                 # too long for the chip: no resident configuration
+    ens = binding.Ensemble(N + 8, 1, path=1)               # ... and for the persistent kernel: the generic kernels take over
+    assert ens.path[0] == 3
