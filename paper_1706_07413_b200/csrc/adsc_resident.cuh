@@ -30,7 +30,7 @@ struct ResParams {
     ResConsts k;
 };
 
-// Shared-memory map of the generation-3 kernel (doubles); the kernel is in adsc_resident3.cuh.
+// Shared-memory map of the resident kernel (doubles); the kernel is in adsc_resident3.cuh.
 template <int P, int THREADS, bool ACC_REG, int CL>
 struct Res3Layout {
     static constexpr int SEG = P * THREADS;

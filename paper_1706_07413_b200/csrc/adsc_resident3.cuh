@@ -1,10 +1,11 @@
-// adsc_resident3.cuh — resident RK4 kernel, third generation ("v3"): one ensemble member per CTA
-// (or per cluster of CL CTAs), the whole state on chip across all RK stages and steps.
+// adsc_resident3.cuh — the resident Runge-Kutta kernel: one ensemble member per CTA (or per cluster of CL CTAs),
+// the whole state on chip across all RK stages and steps.  (Instantiated in adsc_resident3_{a,b,c,d}.cu; host side in
+// adsc_resident.cu.)
 //
 // Arithmetic per stage: telescoped delta rule, two synchronisation points per RK
-// stage, one full exp per thread and short relative polynomials for the other points.  What changed
-// against the earlier generations (generation 1 is adsc_resident.cu; generation 2, same arithmetic with
-// cluster barriers, was removed), and why:
+// stage, one full exp per thread and short relative polynomials for the other points.  Design decisions
+// (against the two earlier generations of this kernel, both removed: "v1" with three cluster barriers per stage, "v2"
+// with the same arithmetic as this one but cluster barriers), and why:
 //   * Synchronisation is point-to-point.  Every sync point is an mbarrier in each CTA's shared memory:
 //     one elected lane per warp arrives on it (split arrive / wait, so the independent arithmetic
 //     placed between them overlaps the skew between warps also inside ONE CTA), and data for other
@@ -16,8 +17,8 @@
 //     coefficients in __constant__ memory, so fp64 instructions take them as c[][] operands: v2
 //     re-materialised ~70 64-bit immediates per thread and stage with IMAD.MOV (8.7 % of all
 //     instructions) and had no register to spare.
-//   * The member-level scan step is a branch-free, fully unrolled, predicated sum of the published warp
-//     totals (two dependent-add chains) instead of a loop of dependent shared-memory loads.
+//   * On 1 or 2 CTAs the member-level scan step is a branch-free, fully unrolled, predicated sum of the published
+//     warp totals (two dependent-add chains) instead of a loop of dependent shared-memory loads.
 //   * The cluster size is a template parameter: any size 1..8 and 16 (the non-portable maximum: 16 x 2048 points
 //     hold the paper's production grid of 2^15 points).
 //   * The member-level scan step leaves the critical path: the exponents of a thread's points are formed WITHOUT
