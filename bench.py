@@ -73,6 +73,8 @@ def parse():
     ap.add_argument("--e2e-parts", type=int, default=8, help="sub-batches (handles, streams) of the e2e leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--spread", action="store_true",
+                    help="ADSC_OPT_SPREAD: latency mode for ensembles that do not fill the device (more, shorter CTAs per member)")
     ap.add_argument("--mode-energies", type=int, default=0, metavar="J",
                     help="also time adsc_mode_energies(J) (SURVEY.md 8(f) f3) on the evolved ensemble and add a "
                          "`mode_energies` object with its own roofline to the line")
@@ -282,7 +284,7 @@ def main():
     Pi_h = torch.from_numpy(np.ascontiguousarray(Pi_all)).pin_memory()
     del Phi_all, Pi_all
 
-    ens = binding.Ensemble(N, B, device=dev, path=args.path, 
+    ens = binding.Ensemble(N, B, device=dev, path=args.path, spread=args.spread,
                            fixed_background=args.fixed_background, rk_order=(args.rk_order if args.rk_order != 4 else None))
     path, cluster = ens.path
     Phi_d, Pi_d = Phi_h.to(dev), Pi_h.to(dev)
@@ -358,7 +360,7 @@ def main():
     # The user-facing way to run a batch from host memory: sub-batches on their own handles and streams, so that one
     # sub-batch's transfers overlap the other's kernels (binding.PipelinedEnsemble; members are independent).
     parts = max(1, min(args.e2e_parts, B // 32))
-    pe = binding.PipelinedEnsemble(N, B, parts=parts, device=dev, path=args.path, 
+    pe = binding.PipelinedEnsemble(N, B, parts=parts, device=dev, path=args.path, spread=args.spread,
                                    fixed_background=args.fixed_background,
                                    rk_order=(args.rk_order if args.rk_order != 4 else None))
     for _ in range(1):
@@ -449,7 +451,7 @@ def main():
         "config": {"workload": WORKLOAD_DESC[name], "N": N, "batch_per_gpu": B, "global_batch": B * world,
                    "rk4_per_step": rk4, "courant": 0.25, "ko_eps": 0.1, "fixed_background": bool(args.fixed_background), "rk_order": args.rk_order,
                    "path": {1: "streaming-persistent", 2: "resident", 3: "streaming-generic"}[path],
-                   "ctas_per_member": cluster,
+                   "ctas_per_member": cluster, "spread": bool(args.spread),
                    "parallelism": f"members sharded over {world} GPU(s), no collective",
                    "l2": "flushed between timed iterations (256 MiB fill)",
                    "active_fraction": active_frac, "masked_fraction_forced": args.masked_fraction},

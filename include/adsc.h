@@ -77,6 +77,14 @@ extern "C" {
                                           All three step paths implement them (the fixed-background
                                           build is RK4 only).  Set it before adsc_bind.            */
 
+#define ADSC_OPT_SPREAD              9  /* 1: latency mode for ensembles that do not fill the device: the resident path cuts
+                                          every member into more, shorter CTAs (clusters of up to 8 CTAs of at least 256
+                                          points) as long as all clusters of the ensemble are still co-resident, so that
+                                          more SMs work on each member (one member of N = 1025: 4 CTAs, 3.8 instead of
+                                          4.5 microseconds per RK4 step).  Same arithmetic, same results up to the order
+                                          of the scan sums.  Default 0 (widest segment: best throughput for ensembles
+                                          that fill the device).  Set it before adsc_bind.                          */
+
 typedef struct adsc_ctx *adsc_handle;
 
 /* One record per member, filled by adsc_diagnostics (host memory). */

@@ -22,6 +22,7 @@ ADSC_OPT_PATH = 3
 ADSC_OPT_STEPS_PER_LAUNCH = 4
 ADSC_OPT_FIXED_BACKGROUND = 7
 ADSC_OPT_RK_ORDER = 8
+ADSC_OPT_SPREAD = 9
 PATH_AUTO, PATH_STREAM, PATH_RESIDENT = 0, 1, 2
 ADSC_PROBE_FP64_FMA, ADSC_PROBE_SHARED_LOAD = 0, 1
 
@@ -197,7 +198,7 @@ class Ensemble:
 
     def __init__(self, N, batch, courant=0.25, ko_eps=0.1, device="cuda:0", stream=None,
                  path=PATH_AUTO, threshold=None, a_resolve_period=None, steps_per_launch=None,
-                 fixed_background=False, rk_order=None):
+                 fixed_background=False, rk_order=None, spread=False):
         import torch
         load_library()
         if not torch.cuda.is_available():
@@ -211,6 +212,8 @@ class Ensemble:
                 adsc_set_option(self.h, ADSC_OPT_FIXED_BACKGROUND, 1)
             if rk_order is not None:
                 adsc_set_option(self.h, ADSC_OPT_RK_ORDER, rk_order)
+            if spread:
+                adsc_set_option(self.h, ADSC_OPT_SPREAD, 1)
             if path != PATH_AUTO:
                 adsc_set_option(self.h, ADSC_OPT_PATH, path)
             if threshold is not None:

@@ -103,6 +103,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->pb.thr = 0.0078125;   // 2^-7 (BASELINE.json configs[1])
     c->pb.fixed_bg = 0;
     c->rk_order = 4;
+    c->spread = 0;
     c->K_A = 0; c->path_opt = 0; c->steps_per_launch = 0;
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
@@ -176,6 +177,12 @@ int adsc_set_option(adsc_handle h, int key, double value)
         h->rk_order = (int)value;
         resolve_path(h);                 // (the fixed-background build of the resident kernel is RK4 only)
         if (h->path == 0) { h->path_opt = 0; resolve_path(h); }
+        return ADSC_OK;
+    case ADSC_OPT_SPREAD:
+        if (!(value == 0.0 || value == 1.0)) return fail(h, ADSC_EINVAL, "spread: 0 or 1");
+        if (h->bound) return fail(h, ADSC_ESTATE, "set ADSC_OPT_SPREAD before adsc_bind");
+        h->spread = (int)value;
+        resolve_path(h);
         return ADSC_OK;
     default:
         return fail(h, ADSC_EINVAL, "unknown option key");

@@ -94,6 +94,7 @@ struct adsc_ctx {
     bool sp_ok;              // persistent streaming kernel usable (decided at adsc_bind)
     int sp_G, sp_groups, sp_SQ;   // chunks per member, concurrent members, 256-point slices per chunk
     int sms_hint;            // SM count assumed for the layout (the device's if one was visible at adsc_create, else 148)
+    int spread;              // ADSC_OPT_SPREAD: narrower segments for ensembles that do not fill the device
     int rk_order;            // 4 (classical RK4, default), 3 (Heun's third-order rule) or 2 (explicit midpoint): R12, R25
     std::string err;
 };

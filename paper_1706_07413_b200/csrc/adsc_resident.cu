@@ -13,17 +13,23 @@ static const void *fn_big(int cl, int kind)
     if (const void *f = res3_big_b(cl, kind)) return f;
     return res3_big_c(cl, kind);
 }
-static const void *fn_1024(int cl, int kind) { return cl == 1 ? res3_small(1024, kind) : res3_small_odd(1024, cl, kind); }
-static const void *fn_512(int cl, int kind) { return cl == 1 ? res3_small(512, kind) : res3_small_odd(512, cl, kind); }
-static const void *fn_256(int cl, int kind) { return cl == 1 ? res3_small(256, kind) : res3_small_odd(256, cl, kind); }
+static const void *fn_short(int seg, int cl, int kind)
+{
+    if (cl == 1) return res3_small(seg, kind);
+    if (const void *f = res3_small_odd(seg, cl, kind)) return f;
+    return res3_small_even(seg, cl, kind);
+}
+static const void *fn_1024(int cl, int kind) { return fn_short(1024, cl, kind); }
+static const void *fn_512(int cl, int kind) { return fn_short(512, cl, kind); }
+static const void *fn_256(int cl, int kind) { return fn_short(256, cl, kind); }
 static const void *fn_128(int cl, int kind) { return cl == 1 ? res3_small(128, kind) : res3_small_odd(128, cl, kind); }
 
 // widest segment first
 static const ResConfig g_cfgs[] = {
     { "P8xT256", 8, 256, 2048, true, Res3Layout<8, 256, true, RES_MAX_CLUSTER>::bytes, fn_big },   // N-1 = cl x 2048, cl in 1..8, 16
-    { "P8xT128", 8, 128, 1024, false, Res3Layout<8, 128, false, 7>::bytes, fn_1024 },                // cl = 1, 3, 5, 7
-    { "P4xT128", 4, 128, 512, false, Res3Layout<4, 128, false, 7>::bytes, fn_512 },
-    { "P4xT64", 4, 64, 256, false, Res3Layout<4, 64, false, 7>::bytes, fn_256 },
+    { "P8xT128", 8, 128, 1024, false, Res3Layout<8, 128, false, 8>::bytes, fn_1024 },                // cl = 1..5, 7, 8
+    { "P4xT128", 4, 128, 512, false, Res3Layout<4, 128, false, 8>::bytes, fn_512 },
+    { "P4xT64", 4, 64, 256, false, Res3Layout<4, 64, false, 8>::bytes, fn_256 },
     { "P4xT32", 4, 32, 128, false, Res3Layout<4, 32, false, 7>::bytes, fn_128 },
 };
 constexpr int n_cfgs = sizeof(g_cfgs) / sizeof(g_cfgs[0]);
@@ -37,12 +43,16 @@ static int kind_of(const adsc_ctx *c)
 const char *resident_cfg_name(int cfg) { return (cfg >= 0 && cfg < n_cfgs) ? g_cfgs[cfg].name : "none"; }
 
 // Pick the widest segment that tiles N-1 with a cluster size the kernel is compiled for (1..8 CTAs per member, or
-// 16, the non-portable maximum).  Returns false if no resident configuration holds N.
+// 16, the non-portable maximum).  With ADSC_OPT_SPREAD and an ensemble that does not fill the device, the NARROWEST
+// segment of at least 256 points whose clusters (at most 8 CTAs) still all fit on the device at once: more SMs per
+// member, shorter steps.  Returns false if no resident configuration holds N.
 bool resident_select(adsc_ctx *c)
 {
     const int n_act = c->pb.N - 1;
     const int kind = kind_of(c);
     if (kind < 0) return false;
+    const int sms = c->dev_sms > 0 ? c->dev_sms : c->sms_hint;
+    int pick = -1, pick_cl = 0;
     for (int k = 0; k < n_cfgs; ++k) {
         const ResConfig &g = g_cfgs[k];
         if (n_act % g.seg) continue;
@@ -50,10 +60,13 @@ bool resident_select(adsc_ctx *c)
         if (cl < 1 || cl > RES_MAX_CLUSTER) continue;
         if (!g.fn(cl, kind)) continue;
         if (c->dev_smem_optin > 0 && g.smem > (size_t)c->dev_smem_optin) continue;
-        c->res_cfg = k; c->cluster = cl;
-        return true;
+        if (pick < 0) { pick = k; pick_cl = cl; if (!c->spread) break; continue; }      // the default: widest segment
+        // spread: a narrower segment, as long as every member's cluster has its own SMs
+        if (g.seg >= 256 && cl <= 8 && (long long)c->pb.B * cl <= sms) { pick = k; pick_cl = cl; }
     }
-    return false;
+    if (pick < 0) return false;
+    c->res_cfg = pick; c->cluster = pick_cl;
+    return true;
 }
 
 // Attributes and launch configuration of the selected kernel (shared by the launch and the check at adsc_bind).

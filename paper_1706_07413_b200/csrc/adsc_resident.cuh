@@ -66,11 +66,12 @@ struct ResConfig {
 };
 constexpr int RES_MAX_CLUSTER = 16;       // non-portable cluster size (8 is the portable limit)
 
-// kernels are instantiated in adsc_resident3_{a,b,c,d}.cu
+// kernels are instantiated in adsc_resident3_{a,b,c,d,e}.cu
 const void *res3_big_a(int cl, int kind);     // 8 points x 256 threads: clusters of 1, 2, 4
 const void *res3_big_b(int cl, int kind);     // ... of 8, 16
 const void *res3_big_c(int cl, int kind);     // ... of 3, 5, 6, 7
 const void *res3_small(int seg, int kind);    // one CTA per member: segments of 1024, 512, 256, 128 points
 const void *res3_small_odd(int seg, int cl, int kind);   // clusters of 3, 5, 7 of those segments (adsc_resident3_d.cu)
+const void *res3_small_even(int seg, int cl, int kind);  // clusters of 2, 4, 8 of 1024, 512, 256 points (adsc_resident3_e.cu)
 
 }  // namespace adsc

@@ -713,3 +713,29 @@ def test_maximum_sizes(env):
         binding.Ensemble(N + 8, 1, path=2)                 # too long for the chip: no resident configuration
     ens = binding.Ensemble(N + 8, 1, path=1)               # ... and for the persistent kernel: the generic kernels take over
     assert ens.path[0] == 3
+
+
+@pytest.mark.parametrize("name,B,N,expect,kw", [
+    ("cfg1", 1, 1025, 4, {}),                          # one member: 4 CTAs of 256 points instead of 1 of 1024
+    ("cfg5", 16, 2049, 8, {}),                         # 16 members: 8 x 256 each (128 SMs)
+    ("cfg5", 40, 2049, 2, dict(rk_order=3)),           # 40 members: 2 x 1024 (80 SMs); 4 x 512 would not be co-resident
+    ("cfg2", 2, 4097, 8, {}),                          # 8 x 512
+    ("cfg5", 200, 2049, 1, {}),                        # the ensemble fills the device: the default choice
+    ("cfg2", 3, 1537, 3, dict(fixed_background=True)),  # 3 x 512 is the only tiling
+])
+def test_spread_option_matches_oracle(env, name, B, N, expect, kw):
+    """ADSC_OPT_SPREAD (latency mode): more, shorter CTAs per member while all clusters stay co-resident."""
+    Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
+    ens, f, d = _gpu_run(env, Phi, Pi, 500, spread=True, **kw)
+    assert ens.path == (2, expect)
+    okw = dict(fixed_background=True) if kw.get("fixed_background") else {}
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 16), rk_order=kw.get("rk_order", 4), **okw).step(500)
+    if kw.get("fixed_background"):
+        assert np.max(np.abs(f["Phi"] - ev.Phi)) <= TOL and np.max(np.abs(f["Pi"] - ev.Pi)) <= TOL
+    else:
+        _compare(f, ev)
+        _bc_invariants(f)
+    assert (d["steps_done"] == 500).all()
+    binding = env["binding"]
+    lib = binding.load_library()
+    assert lib.adsc_set_option(ens.h, binding.ADSC_OPT_SPREAD, 1.0) == binding.ADSC_ESTATE       # after bind
