@@ -739,3 +739,16 @@ def test_spread_option_matches_oracle(env, name, B, N, expect, kw):
     binding = env["binding"]
     lib = binding.load_library()
     assert lib.adsc_set_option(ens.h, binding.ADSC_OPT_SPREAD, 1.0) == binding.ADSC_ESTATE       # after bind
+
+
+def test_run_config_driver(env):
+    """paper_1706_07413_b200/run_config.py (a whole BASELINE config on the GPU): a short window of cfg1 against the
+    oracle's diagnostics."""
+    from paper_1706_07413_b200 import run_config
+    r = run_config.run("cfg1", steps=300, chunk_steps=128)
+    Phi, Pi, _ = env["inputs"].make("cfg1")
+    ev = env["oracle"].Evolution(Phi, Pi).step(300)
+    od = ev.diagnostics()
+    assert r["steps"] == 300 and r["collapsed"] == 0 and r["members"] == 1 and r["path"][0] == 2
+    assert abs(r["min_A"] - od["min_A"][0]) <= TOL
+    assert r["max_rel_mass_drift"] < 1e-6 and r["updates_per_s"] > 0
