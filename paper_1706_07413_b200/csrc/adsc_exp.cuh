@@ -49,7 +49,9 @@ __device__ __forceinline__ double exp3_ref(double x)
 // reference argument only (and to every argument if full evaluations are needed) -- the caller may have `shift`
 // ready much later than x.
 // tier (self-test only): 0, 1, 2 = 2, 3, 5 terms of t; 3 = a full evaluation per point.
-template <int P, bool SCALED = false, bool SHIFTED = false>
+// WARP: the number of terms is chosen for the whole warp (the largest spread of its 32 threads), so that the warp does
+// not execute two branches one after the other when its lanes disagree; every lane of the warp must make the call.
+template <int P, bool SCALED = false, bool SHIFTED = false, bool WARP = false>
 __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], const double scale = 1.0, int *tier = nullptr,
                                           const double shift = 0.0)
 {
@@ -63,6 +65,9 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], 
         big |= (hz > 0x3f900000) ? 1 : 0;    // |z| > 2^-6 (or NaN)
         mid |= (hz > 0x3f500000) ? 1 : 0;    // |z| > 2^-10
         sml |= (hz > 0x3f100000) ? 1 : 0;    // |z| > 2^-14
+    }
+    if (WARP) {
+        sml = __any_sync(0xffffffffu, sml); mid = __any_sync(0xffffffffu, mid); big = __any_sync(0xffffffffu, big);
     }
     const double xs = SHIFTED ? xr + shift : xr;
     const double Er = SCALED ? exp3_ref(xs) * scale : exp3_ref(xs);

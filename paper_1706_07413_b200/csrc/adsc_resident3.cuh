@@ -321,7 +321,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS * P <= 1024) ? 2 : 1) k_resi
                         nd[p] = fma(K.hh, s2, loc);
                     }
                 }
-                exp3_near<P, false, true>(nd, E, 1.0, nullptr, K.hh * B);
+                exp3_near<P, false, true, true>(nd, E, 1.0, nullptr, K.hh * B);
             }
             // a3 fluxes
             double H[P], F[P], kAv[P], G1 = 0.0, G2 = 0.0, Gl1 = 0.0, Gl2 = 0.0;

@@ -539,8 +539,8 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                             loc = fma(-K.c1, f_lo, loc);
                             nd[p] = fma(K.hh, s2 + B, loc);
                         }
-                        if (defer) exp3_near<P>(nd, E);
-                        else exp3_near<P, true>(nd, E, Cst);
+                        if (defer) exp3_near<P, false, false, true>(nd, E);
+                        else exp3_near<P, true, false, true>(nd, E, Cst);
                     }
                     // global operands of the A update (needed at the end of phase 1)
                     double unA[P], acA[P];
