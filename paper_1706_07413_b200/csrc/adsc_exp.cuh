@@ -57,18 +57,16 @@ __device__ __forceinline__ void exp3_near(const double (&x)[P], double (&E)[P], 
 {
     const double xr = x[P - 1];
     double z[P];
-    int big = 0, mid = 0, sml = 0;
+    int hmax = 0;                            // largest |z| of the thread (of the warp), as the high word of the double
 #pragma unroll
     for (int p = 0; p < P - 1; ++p) {
         z[p] = x[p] - xr;
-        const int hz = __double2hiint(z[p]) & 0x7fffffff;
-        big |= (hz > 0x3f900000) ? 1 : 0;    // |z| > 2^-6 (or NaN)
-        mid |= (hz > 0x3f500000) ? 1 : 0;    // |z| > 2^-10
-        sml |= (hz > 0x3f100000) ? 1 : 0;    // |z| > 2^-14
+        hmax = max(hmax, __double2hiint(z[p]) & 0x7fffffff);
     }
-    if (WARP) {
-        sml = __any_sync(0xffffffffu, sml); mid = __any_sync(0xffffffffu, mid); big = __any_sync(0xffffffffu, big);
-    }
+    if (WARP) hmax = __reduce_max_sync(0xffffffffu, hmax);
+    const int big = hmax > 0x3f900000;       // |z| > 2^-6 (or NaN)
+    const int mid = hmax > 0x3f500000;       // |z| > 2^-10
+    const int sml = hmax > 0x3f100000;       // |z| > 2^-14
     const double xs = SHIFTED ? xr + shift : xr;
     const double Er = SCALED ? exp3_ref(xs) * scale : exp3_ref(xs);
     E[P - 1] = Er;
