@@ -174,6 +174,39 @@ int adsc_get_fields_host_async(adsc_handle h, double *h_Phi, double *h_Pi, doubl
  * or a NULL pointer, ESTATE before adsc_set_initial. */
 int adsc_mode_energies(adsc_handle h, int J, double *host_out);
 
+/* The same spectrum for callers that are not allowed to allocate GPU memory, and have none to spare for a workspace.
+ * Who that is: a program that gave the whole GPU to its own memory pool when it started (a training or serving
+ * process with a caching allocator, a client running under a fixed per-process memory limit), so that a cudaMalloc
+ * made behind its back fails or breaks its accounting; and code on a latency-critical path, where cudaMalloc and
+ * cudaFree are ruled out because they stall the whole device while they run.  Such a caller can still pass its own
+ * arrays, so this entry point takes the fields and the result as plain device pointers, needs no handle and no
+ * workspace, and keeps the one thing the computation needs beyond them, the per-slice partial sums of the two
+ * kernels, in an array of ADSC_STATIC_SCRATCH_BYTES that is built into the library.  It calls no cudaMalloc, no
+ * cudaFree and no library routine that allocates.
+ *   d_Phi, d_Pi  DEVICE pointers, [batch][N] doubles row-major, 8-byte aligned, read only.  Phi_{N-1}, Pi_{N-1} and
+ *                Phi_0 do not enter (the integrands vanish there), so the result equals adsc_mode_energies of a
+ *                handle whose state was set from the same two arrays.
+ *   d_E          DEVICE pointer, [batch][J] doubles, written.
+ *   cuda_stream  a cudaStream_t cast to void* (NULL = legacy default stream) on the device that is current at the
+ *                call; the pointers must belong to that device.  Two kernels are enqueued; the call does not wait.
+ * Limits: N odd and >= 9, 1 <= J <= 32, J <= N/4, and batch * J <= ADSC_STATIC_SCRATCH_BYTES / 16 (= 131072; e.g.
+ * 4096 members at J = 32).  Beyond that the call returns ADSC_EINVAL and says so in adsc_last_error(NULL); cut the
+ * batch into pieces or use adsc_mode_energies.  The price of the built-in array: every GPU on which the library's
+ * code gets loaded holds those 2 MiB until the process ends, whether or not this function is ever called.
+ * First call on each device: it looks up where the built-in array lives on that device (cudaGetSymbolAddress, which
+ * may also be the moment the CUDA runtime loads the library's code there) and remembers it.  Make that first call
+ * during start-up, before any stream capture is begun; later calls only launch the two kernels.
+ * Sharing: there is ONE such array per device and every call on that device uses it, whatever the stream or thread.
+ * Each call overwrites all the slots it later reads, so nothing has to be cleared and stale contents of the previous
+ * call are harmless; but two calls whose kernels can run at the same time on one device (different streams, no
+ * event between them) write the same slots and corrupt each other.  Keep the calls of one device on one stream, or
+ * order them with events.
+ * Errors: ADSC_EINVAL (arguments, limit), ADSC_ECUDA (no device, launch failure); text from adsc_last_error(NULL) on
+ * the calling thread.  (R19, R24.) */
+#define ADSC_STATIC_SCRATCH_BYTES (2u << 20)
+int adsc_mode_energies_static(int N, int batch, int J, const double *d_Phi, const double *d_Pi, double *d_E,
+                              void *cuda_stream);
+
 /* Roofline denominators measured on the current CUDA device ("a DFMA issue-rate probe and a
  * shared-memory bandwidth probe"; none of the method's arithmetic).  kind ADSC_PROBE_FP64_FMA: *result = flop/s of
  * independent FP64 fused multiply-adds on every SM (2 flop each); ADSC_PROBE_SHARED_LOAD: *result = bytes/s of

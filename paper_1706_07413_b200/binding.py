@@ -62,6 +62,7 @@ _SIGS = {
     "adsc_set_initial_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_get_fields_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_mode_energies": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "adsc_mode_energies_static": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_get_fields_host_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "adsc_launch_count": (C.c_longlong, [C.c_void_p]),
     "adsc_path": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
@@ -154,6 +155,11 @@ def adsc_get_fields_host(h, h_Phi, h_Pi, h_A, h_delta):
 
 def adsc_mode_energies(h, J, host_out_ptr):
     _check(h, load_library().adsc_mode_energies(h, int(J), host_out_ptr))
+
+
+def adsc_mode_energies_static(N, batch, J, d_Phi, d_Pi, d_E, cuda_stream):
+    """Forward to the entry point that allocates nothing (scratch built into the library); device pointers."""
+    _check(None, load_library().adsc_mode_energies_static(int(N), int(batch), int(J), d_Phi, d_Pi, d_E, cuda_stream))
 
 
 def adsc_get_fields_host_async(h, h_Phi, h_Pi, h_A, h_delta):

@@ -14,6 +14,9 @@ static thread_local std::string g_create_error = "";   // per calling thread: ad
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// For entry points that take no handle: the text adsc_last_error(NULL) returns on this thread.
+void adsc::set_thread_error(const std::string &msg) { g_create_error = msg; }
+
 static void compute_layout(adsc_ctx *c)
 {
     Layout &L = c->lay;

@@ -114,6 +114,8 @@ inline void rk_tableau(int order, double dt, double a_next[4], double b_w[4])
     }
 }
 
+void set_thread_error(const std::string &msg);               // adsc_api.cu: message for adsc_last_error(NULL) on this thread
+
 // ---- launchers implemented in the .cu files (all asynchronous on ctx->stream) -----------
 cudaError_t launch_tables(adsc_ctx *c);
 cudaError_t launch_pack(adsc_ctx *c, const double *src, int field, bool init_rec);
