@@ -99,16 +99,24 @@ __device__ __forceinline__ double ld_cg(const double *p)
     return v;
 }
 
-// One 16-byte mailbox slot {value, stamp}: a single 128-bit transaction each way (STG/LDG.E.128.STRONG.GPU), so a
-// reader that sees the stamp of the round also sees the value that was written with it.
+// One 16-byte mailbox slot {value, stamp}, written and read as ONE scalar 128-bit access (PTX type .b128, relaxed, gpu
+// scope; SASS STG/LDG.E.128.STRONG.GPU).  The protocol needs a reader that sees the stamp of the round to see the value
+// stored with it, i.e. the 16 bytes must never tear.  A .v2.b64 access would not promise that: the PTX memory model
+// treats a vector access as two separate 64-bit accesses in unspecified order.  A .b128 access is a single scalar
+// operation on a naturally aligned 16-byte location; that such an access is single-copy atomic is what sm_90+ builds
+// its atom.b128 on, and it is the one assumption of this protocol ("mailbox assumption").  Slots are
+// 16-byte aligned by construction: the mailbox region is 256-byte aligned, SA_MBOX is even and slot offsets are even.
+static_assert(SA_MBOX % 2 == 0, "mailbox slots must stay 16-byte aligned");
 __device__ __forceinline__ void st_pair(double *p, double v, unsigned long long w)
 {
-    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(p), "l"(__double_as_longlong(v)), "l"(w) : "memory");
+    asm volatile("{\n\t.reg .b128 q;\n\tmov.b128 q, {%1, %2};\n\tst.relaxed.gpu.global.b128 [%0], q;\n\t}"
+                 ::"l"(p), "l"(__double_as_longlong(v)), "l"(w) : "memory");
 }
 __device__ __forceinline__ void ld_pair(const double *p, double &v, unsigned long long &w)
 {
     long long a;
-    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(w) : "l"(p) : "memory");
+    asm volatile("{\n\t.reg .b128 q;\n\tld.relaxed.gpu.global.b128 q, [%2];\n\tmov.b128 {%0, %1}, q;\n\t}"
+                 : "=l"(a), "=l"(w) : "l"(p) : "memory");
     v = __longlong_as_double(a);
 }
 
