@@ -53,7 +53,10 @@ extern "C" {
                                           coefficient tables staged by bulk asynchronous
                                           copies, u^n and accumulator in global memory; it
                                           needs N-1 to be a multiple of 8 and all CTAs of a
-                                          member co-resident, and falls back to 3 otherwise);
+                                          member co-resident, and falls back to 3 otherwise;
+                                          its layout depends on the SM count of the device that
+                                          is current at adsc_create: adsc_bind on a device with
+                                          another SM count returns ESTATE when 1 was forced);
                                           2 force the resident (shared-memory/register)
                                           kernel, EINVAL if it cannot hold N; 3 force the
                                           generic streaming kernels (one launch per phase,
@@ -83,7 +86,9 @@ extern "C" {
                                           more SMs work on each member (one member of N = 1025: 4 CTAs, 3.8 instead of
                                           4.5 microseconds per RK4 step).  Same arithmetic, same results up to the order
                                           of the scan sums.  Default 0 (widest segment: best throughput for ensembles
-                                          that fill the device).  Set it before adsc_bind.                          */
+                                          that fill the device).  Set it before adsc_bind; adsc_bind asks the device
+                                          how many clusters it really holds at once and steps back to wider segments
+                                          until all members' clusters are co-resident (adsc_path tells the outcome). */
 
 typedef struct adsc_ctx *adsc_handle;
 

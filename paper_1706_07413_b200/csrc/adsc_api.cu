@@ -41,8 +41,7 @@ static void compute_layout(adsc_ctx *c)
     L.off_tab = off; off += align_up((size_t)5 * (c->pb.NP + 2 * HAL) * sizeof(double), 256);
     L.off_tabp = off; off += (c->path == 1) ? align_up((size_t)3 * c->pb.NP * sizeof(double), 256) : 0;
     L.off_rec = off; off += align_up((size_t)c->pb.B * sizeof(MemberRec), 256);
-    L.off_mbox = off; off += align_up((size_t)SP_MAX_CTAS * 2 * 24 * sizeof(double), 256);
-    L.off_cnt = off; off += align_up((size_t)SP_MAX_CTAS * sizeof(unsigned long long), 256);
+    L.off_mbox = off; off += align_up((size_t)SP_MAX_CTAS * 2 * SA_MBOX * sizeof(double), 256);   // [groups][2][G][SA_MBOX], groups * G <= SP_MAX_CTAS
     L.total = off;
 }
 
@@ -106,7 +105,7 @@ adsc_handle adsc_create(int N, int batch, double courant, double ko_eps)
     c->pb.thr = 0.0078125;   // 2^-7 (BASELINE.json configs[1])
     c->pb.fixed_bg = 0;
     c->rk_order = 4;
-    c->spread = 0;
+    c->spread = 0; c->spread_cap = 8;
     c->K_A = 0; c->path_opt = 0; c->steps_per_launch = 0;
     c->bound = false; c->have_state = false; c->stream = nullptr; c->ws_base = nullptr;
     c->launches = 0; c->global_step = 0; c->dev_sms = 0; c->dev_smem_optin = 0;
@@ -227,18 +226,26 @@ int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream)
     h->ws.tab = (double *)(base + L.off_tab);
     h->ws.rec = (MemberRec *)(base + L.off_rec);
     h->ws.sp_mbox = (double *)(base + L.off_mbox);
-    h->ws.sp_counter = (unsigned long long *)(base + L.off_cnt);
     h->ws.tabp = (double *)(base + L.off_tabp);
     // the persistent streaming kernel needs every CTA of a member co-resident on THIS device and the row pitch the
     // layout was made for; otherwise one kernel per phase (which takes any pitch)
     if (h->path == 1) {
         int G = 0, SQ = 0, groups = 0;
-        if (!stream_async_select(h->pb.N, h->pb.B, h->dev_sms, &G, &SQ, &groups) || sa_row_pitch(h->pb.N, G, SQ) != h->pb.NP) { h->path = 3; h->sp_ok = false; }
+        if (!stream_async_select(h->pb.N, h->pb.B, h->dev_sms, &G, &SQ, &groups) || sa_row_pitch(h->pb.N, G, SQ) != h->pb.NP) {
+            // The layout (and adsc_workspace_bytes) was made for the SM count seen at adsc_create.  Asked for by name,
+            // the persistent kernel is not quietly replaced by the three-launches-per-stage kernels: say what to do.
+            if (h->path_opt == 1)
+                return fail(h, ADSC_ESTATE, "ADSC_OPT_PATH = 1 was chosen for a device with " + std::to_string(h->sms_hint)
+                            + " SMs but adsc_bind runs on one with " + std::to_string(h->dev_sms)
+                            + ": call adsc_create with the device that will be bound current (cudaSetDevice first)");
+            h->path = 3; h->sp_ok = false;
+        }
         else { h->sp_G = G; h->sp_SQ = SQ; h->sp_groups = groups; }
     }
     // the resident configuration was chosen at adsc_create without a device: make sure THIS device can hold one
     // cluster of it (shared-memory opt-in, cluster size)
     if (h->path == 2) {
+        if (h->spread && h->spread_cap != 8) { h->spread_cap = 8; (void)resident_select(h); }   // (a re-bind: start over)
         int clusters = 0;
         const cudaError_t e = resident_check(h, &clusters);
         if (e != cudaSuccess || clusters < 1) {
@@ -247,6 +254,20 @@ int adsc_bind(adsc_handle h, void *d_workspace, size_t bytes, void *cuda_stream)
                         + std::to_string(h->cluster) + " CTAs per member) cannot run on this device"
                         + (e != cudaSuccess ? std::string(": ") + cudaGetErrorString(e) : std::string())
                         + "; set ADSC_OPT_PATH to 1 (streaming) before adsc_bind");
+        }
+        // ADSC_OPT_SPREAD promises that all clusters of the ensemble are co-resident.  B * cluster <= SMs (the test
+        // resident_select applies without a device) does not guarantee it: a cluster must sit inside one GPC, so the
+        // device may hold fewer.  Step back to the next wider segment until the occupancy query agrees (the widest one,
+        // the default, ends the loop at the latest).  The layout does not depend on the segment.
+        while (h->spread && clusters < h->pb.B) {
+            const int before = h->cluster;
+            h->spread_cap = before - 1;
+            if (h->spread_cap < 1 || !resident_select(h) || h->cluster == before) break;
+            const cudaError_t e2 = resident_check(h, &clusters);
+            if (e2 != cudaSuccess || clusters < 1) {
+                (void)cudaGetLastError();
+                return fail(h, ADSC_ECUDA, std::string("the resident kernel (") + resident_cfg_name(h->res_cfg) + ") cannot run on this device");
+            }
         }
     }
     const size_t NT = (size_t)h->pb.NP + 2 * HAL;
@@ -417,8 +438,11 @@ int adsc_mode_energies(adsc_handle h, int J, double *host_out)
     if (!host_out) return fail(h, ADSC_EINVAL, "null output");
     if (J < 1 || J > 32 || 4 * J > h->pb.NP) return fail(h, ADSC_EINVAL, "J must be in 1..32 (and <= N/4)");
     double *d_out = h->ws.Ac;                    // scratch: [B][NP] doubles: [B][J] results, then the slice partials
-    const size_t used = ((size_t)h->pb.B * J + 31) / 32 * 32;
-    ADSC_CUDA(launch_mode_energies(h, J, d_out, d_out + used, (size_t)h->pb.B * h->pb.NP - used), "mode projection kernels");
+    // One slice per member needs 2 B J doubles behind the B J results: 3 B J <= B NP follows from 4 J <= NP above, so
+    // the partials always fit in the field (the check below guards the subtraction should that condition ever change).
+    const size_t total = (size_t)h->pb.B * h->pb.NP, used = (size_t)h->pb.B * J;
+    if (total < used + 2 * used) return fail(h, ADSC_EINVAL, "J too large for the scratch field of this N");
+    ADSC_CUDA(launch_mode_energies(h, J, d_out, d_out + used, total - used), "mode projection kernels");
     ADSC_CUDA(cudaMemcpyAsync(host_out, d_out, (size_t)h->pb.B * J * sizeof(double), cudaMemcpyDeviceToHost, h->stream),
               "D2H mode energies");
     ADSC_CUDA(cudaStreamSynchronize(h->stream), "stream synchronize");

@@ -13,7 +13,8 @@ namespace adsc {
 constexpr int HAL = 4;            // table halo on each side (3 used by the widest stencil)
 constexpr int GEN_TILE = 1024;    // points per CTA tile of the streaming kernels
 constexpr int GEN_THREADS = 256;  // 4 points per thread
-constexpr int SP_MAX_CTAS = 1024; // persistent streaming kernel: mailbox / barrier slots in the workspace
+constexpr int SP_MAX_CTAS = 1024; // persistent streaming kernel: at most this many CTAs (groups * G) have a mailbox in the workspace
+constexpr int SA_MBOX = 40;       // ... doubles per chunk mailbox: 17 slots {value, stamp} + padding (adsc_stream_async.cu)
 
 // Per-member record kept on the device (copied to the host by adsc_diagnostics).
 struct MemberRec {
@@ -57,8 +58,7 @@ struct Workspace {
     double *tot2, *carry2;   // tiled constraint solve: tile totals / exclusive prefix of the A integrand
     double *part;        // tiled constraint solve: [B][ntiles][6] diagnostics partials
     double *stage[2];    // host staging [B][N]
-    double *sp_mbox;     // persistent streaming: [SP_MAX_CTAS][2][24] chunk mailboxes
-    unsigned long long *sp_counter;   // persistent streaming: [SP_MAX_CTAS] group barrier counters
+    double *sp_mbox;     // persistent streaming: [groups][2][G][SA_MBOX] chunk mailboxes (room for SP_MAX_CTAS chunks)
     double *tab;         // 5 tables
     double *tabp;        // persistent streaming: -2 sc, tan^2, cot^2/(12h) permuted per 256-point slice [NP/256][3][256]
     MemberRec *rec;      // [B]
@@ -66,7 +66,7 @@ struct Workspace {
 
 struct Layout {
     size_t off_U[3], off_Ua[3], off_Ub[3], off_ACC[3], off_dl, off_Ac, off_tot, off_carry, off_tot2, off_carry2, off_part,
-        off_stage[2], off_tab, off_tabp, off_rec, off_mbox, off_cnt, total;
+        off_stage[2], off_tab, off_tabp, off_rec, off_mbox, total;
     int ntiles;
 };
 
@@ -95,6 +95,7 @@ struct adsc_ctx {
     int sp_G, sp_groups, sp_SQ;   // chunks per member, concurrent members, 256-point slices per chunk
     int sms_hint;            // SM count assumed for the layout (the device's if one was visible at adsc_create, else 148)
     int spread;              // ADSC_OPT_SPREAD: narrower segments for ensembles that do not fill the device
+    int spread_cap;          // ... largest cluster the spread choice may use (8; lowered at adsc_bind when the device holds fewer clusters than members)
     int rk_order;            // 4 (classical RK4, default), 3 (Heun's third-order rule) or 2 (explicit midpoint): R12, R25
     std::string err;
 };

@@ -62,7 +62,7 @@ bool resident_select(adsc_ctx *c)
         if (c->dev_smem_optin > 0 && g.smem > (size_t)c->dev_smem_optin) continue;
         if (pick < 0) { pick = k; pick_cl = cl; if (!c->spread) break; continue; }      // the default: widest segment
         // spread: a narrower segment, as long as every member's cluster has its own SMs
-        if (g.seg >= 256 && cl <= 8 && (long long)c->pb.B * cl <= sms) { pick = k; pick_cl = cl; }
+        if (g.seg >= 256 && cl <= c->spread_cap && (long long)c->pb.B * cl <= sms) { pick = k; pick_cl = cl; }
     }
     if (pick < 0) return false;
     c->res_cfg = pick; c->cluster = pick_cl;

@@ -42,7 +42,7 @@ constexpr int SA_RS = SA_T + 2;           // 16-byte columns per chunk row of a 
 constexpr int SA_RS3 = SA_T / 2 + 2;      // ... of the fourth (half) tile
 constexpr int SA_TS = 4 * SA_RS;          // tile stride
 constexpr int SA_FS = 3 * SA_TS + 4 * SA_RS3;   // field stride (16-byte units)
-constexpr int SA_MBOX = 40;               // doubles per chunk mailbox: 17 slots {value, stamp} + padding
+// (SA_MBOX, the doubles per chunk mailbox, is in adsc_internal.cuh: the workspace layout is sized from it)
 constexpr int SA_SLOT = SA_SL * 8;        // bytes of one table slice
 // The two warps with the fewest slices of a ragged chunk serve the stage: SA_WS scans the slice totals, publishes the
 // chunk total and computes the boundary fluxes (pre-pass); SA_WH exchanges the chunk edges and later gathers the

@@ -374,7 +374,8 @@ def test_tc_sweep_driver_matches_oracle(env):
 # ------------------------------------------------- f3: normal-mode projection diagnostic
 
 @pytest.mark.parametrize("name,B,N,J,nsteps", [("cfg3", 6, 2049, 8, 300), ("cfg2", 3, 4097, 16, 100),
-                                                 ("cfg5", 2, 1025, 32, 0), ("cfg4", 1, 66699, 12, 10)])
+                                                 ("cfg5", 2, 1025, 32, 0), ("cfg4", 1, 66699, 12, 10),
+                                                 ("cfg5", 1, 13, 3, 0), ("cfg5", 2, 29, 7, 0)])   # rows shorter than 32 doubles
 def test_mode_energies_match_oracle(env, name, B, N, J, nsteps):
     """E_j of the evolved state against the oracle's projection of the
     oracle-evolved state; for the two-mode data the spectrum stays in modes 0 and 1 at leading order."""
@@ -721,13 +722,15 @@ def test_maximum_sizes(env):
     ("cfg5", 40, 2049, 2, dict(rk_order=3)),           # 40 members: 2 x 1024 (80 SMs); 4 x 512 would not be co-resident
     ("cfg2", 2, 4097, 8, {}),                          # 8 x 512
     ("cfg5", 200, 2049, 1, {}),                        # the ensemble fills the device: the default choice
+    ("cfg5", 18, 2049, (4, 8), {}),                    # 18 x 8 = 144 SMs, but a cluster of 8 must sit in one GPC: if the
+                                                       # device holds fewer than 18 of them, adsc_bind steps back to 4 x 512
     ("cfg2", 3, 1537, 3, dict(fixed_background=True)),  # 3 x 512 is the only tiling
 ])
 def test_spread_option_matches_oracle(env, name, B, N, expect, kw):
     """ADSC_OPT_SPREAD (latency mode): more, shorter CTAs per member while all clusters stay co-resident."""
     Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
     ens, f, d = _gpu_run(env, Phi, Pi, 500, spread=True, **kw)
-    assert ens.path == (2, expect)
+    assert ens.path[0] == 2 and (ens.path[1] in expect if isinstance(expect, tuple) else ens.path[1] == expect), ens.path
     okw = dict(fixed_background=True) if kw.get("fixed_background") else {}
     ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 16), rk_order=kw.get("rk_order", 4), **okw).step(500)
     if kw.get("fixed_background"):
