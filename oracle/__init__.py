@@ -172,7 +172,7 @@ class Evolution:
         self.Phi, self.Pi, self.A = s["Phi"], s["Pi"], s["A"]
         self.fixed_background = bool(fixed_background)
         self.rk_order = int(rk_order)
-        assert not (self.fixed_background and self.rk_order != 4)
+        assert self.rk_order in (2, 3, 4)
         if self.fixed_background:          # A and delta held fixed at 1 and 0
             self.A = np.ones_like(self.Phi)
         self.B, self.N = self.Phi.shape
@@ -185,6 +185,15 @@ class Evolution:
         self.t_collapse = np.full(self.B, np.nan)
 
     def step(self, nsteps: int):
+        if self.fixed_background and self.rk_order != 4:   # PAPER.md:57 + :177: Table II runs with the third-order rule
+            r = lib().oracle_evolve_fixed_rk(
+                C.c_int(self.N), C.c_int(self.B), C.c_double(self.courant), C.c_double(self.ko_eps),
+                C.c_int(self.rk_order), C.c_longlong(nsteps), _p(self.Phi), _p(self.Pi), _p(self.A),
+                self.steps_done.ctypes.data_as(C.POINTER(C.c_longlong)),
+                self.collapsed.ctypes.data_as(C.POINTER(C.c_int)), _p(self.t_collapse),
+                C.c_int(self.nthreads))
+            assert r == 0
+            return self
         if self.fixed_background:
             r = lib().oracle_evolve_fixed(
                 C.c_int(self.N), C.c_int(self.B), C.c_double(self.courant), C.c_double(self.ko_eps),

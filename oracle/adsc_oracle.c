@@ -568,6 +568,17 @@ int oracle_evolve_rk(int N, int B, double courant, double ko_eps, double thr, in
     return evolve(N, B, courant, ko_eps, thr, K_A, 0, rk_order, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
 }
 
+/* Fixed background (Table II) with the second- or third-order rule: the paper's production runs use the
+ * third-order option, so its Table II timings are fixed-background RK3 evolutions.  Same evolve(), same
+ * rhs(): only the two switches are set together. */
+int oracle_evolve_fixed_rk(int N, int B, double courant, double ko_eps, int rk_order,
+                           long long nsteps, double *Phi, double *Pi, double *A,
+                           long long *steps_done, int *collapsed, double *t_collapse, int nthreads)
+{
+    if (rk_order < 2 || rk_order > 4) return -1;
+    return evolve(N, B, courant, ko_eps, 0.0, 0, 1, rk_order, nsteps, Phi, Pi, A, steps_done, collapsed, t_collapse, nthreads);
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

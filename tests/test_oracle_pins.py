@@ -511,3 +511,51 @@ def test_F6_rk_orders_of_accuracy():
         assert lo < r1 < hi and lo < r2 < hi, (order, errs, r1, r2)
     # the three rules are genuinely different programs: at the same dt their results differ by far more than rounding
     assert np.abs(run(3, 0.2) - run(4, 0.2)).max() > 1e-8
+
+
+def test_F7_fixed_background_rk2_rk3_orders_linearity_and_dissipation_sign():
+    # PAPER.md:57 ("the results presented here use the third-order accurate option") with PAPER.md:177 (Table II:
+    # A = 1, delta = 0 held fixed): the fixed-background evolution under the second- and third-order rules.
+    # (1) order of accuracy at fixed grid, as F6; (2) every step is linear, so scaling the data by a power of two
+    # scales the result bit for bit; (3) A = 1, delta = 0 untouched and nothing collapses; (4) the rules differ from
+    # RK4 and from each other by far more than rounding; (5) the amplification of an exact eigenmode of the
+    # semi-discrete operator over one period is the rule's stability polynomial: for Heun-3 |R(i w dt)| < 1 while for
+    # the midpoint rule |R| > 1, so the linear energy falls under RK3 and grows under RK2 (ko_eps = 0).
+    N, T = 129, 0.6
+    x = inputs.grid(N); tb = oracle.tables(N)
+    e1, de1 = inputs.eigenmode(1, x)
+    Phi0 = 0.3 * de1; Phi0[0] = Phi0[-1] = 0.0
+    Pi0 = inputs.gaussian_Pi(N, 1.0, 0.25)[0]
+    h = (np.pi / 2) / (N - 1)
+    def run(order, lam, scale=1.0):
+        n = int(round(T / (lam * h)))
+        ev = oracle.Evolution(scale * Phi0, scale * Pi0, courant=T / (n * h), ko_eps=0.0, rk_order=order,
+                              fixed_background=True).step(n)
+        assert (ev.A == 1).all() and (ev.delta == 0).all() and not ev.collapsed.any()
+        return np.concatenate([ev.Phi[0], ev.Pi[0]])
+    ref = run(4, 0.00625)
+    # (the linear problem reaches the asymptotic ratio of the third-order rule later than F6's nonlinear one: its
+    # dt^4 term has the opposite sign, so the ratios rise towards 8 from below)
+    for order, lams, lo, hi in ((2, (0.4, 0.2, 0.1), 3.5, 4.6), (3, (0.1, 0.05, 0.025), 6.8, 8.4)):
+        errs = [np.abs(run(order, lam) - ref).max() for lam in lams]
+        r1, r2 = errs[0] / errs[1], errs[1] / errs[2]
+        assert lo < r1 < hi and lo < r2 < hi, (order, errs, r1, r2)
+        assert np.array_equal(run(order, 0.2, scale=2.0 ** -9), run(order, 0.2) * 2.0 ** -9)
+    assert np.abs(run(3, 0.2) - run(4, 0.2)).max() > 1e-8 and np.abs(run(3, 0.2) - run(2, 0.2)).max() > 1e-8
+    # the fixed-background rule is not the dynamical one with a small back-reaction: at this amplitude they differ
+    dyn = oracle.Evolution(Phi0, Pi0, courant=0.2, ko_eps=0.0, rk_order=3).step(50)
+    fix = oracle.Evolution(Phi0, Pi0, courant=0.2, ko_eps=0.0, rk_order=3, fixed_background=True).step(50)
+    assert np.abs(dyn.Phi[0] - fix.Phi[0]).max() > 1e-4
+    def energy(ev):
+        return (tb["w"][:-1] * tb["T"][:-1] * (ev.Phi[0][:-1] ** 2 + ev.Pi[0][:-1] ** 2)).sum()
+    Phi1 = de1.copy(); Phi1[0] = Phi1[-1] = 0.0
+    # |R(iy)|^2 - 1 per step, y = w dt, w = omega_1 = 5: Heun-3 -y^4/12, midpoint +y^4/4; over one period t = pi.
+    # (The midpoint rule amplifies EVERY mode, the grid's highest by (w_max dt)^4/4 per step: at courant 1/4 rounding
+    # noise gains e^3.5 over the 1024 steps, harmless; at 1/2 it would swamp the solution.)
+    for order, courant, sign in ((3, 0.5, -1.0), (2, 0.25, +1.0)):
+        n = int(round(2 * (N - 1) / courant))
+        ev = oracle.Evolution(Phi1, np.zeros(N), courant=courant, ko_eps=0.0, rk_order=order, fixed_background=True)
+        E0 = energy(ev); ev.step(n); E1 = energy(ev)
+        y = 5.0 * courant * h
+        expect = (-(y ** 4) / 12.0 if order == 3 else (y ** 4) / 4.0) * n
+        assert sign * (E1 / E0 - 1.0) > 0 and abs((E1 / E0 - 1.0) / expect - 1.0) < 0.02, (order, E1 / E0 - 1.0, expect)
