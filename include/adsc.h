@@ -77,8 +77,12 @@ extern "C" {
 #define ADSC_OPT_RK_ORDER            8  /* 4 (default): classical RK4; 3: Heun's third-order rule; 2:
                                           explicit midpoint ("second, third, and fourth order accurate
                                           Runge-Kutta"; tableaux are readings R12, R25).
-                                          All three step paths implement them (the fixed-background
-                                          build is RK4 only).  Set it before adsc_bind.            */
+                                          All three step paths implement them.  Together with
+                                          ADSC_OPT_FIXED_BACKGROUND (the paper's Table II runs:
+                                          PAPER.md:57 + :177) orders 3 and 2 are supported on the two
+                                          streaming paths only: the resident kernel has no build of
+                                          that combination, auto then picks a streaming path and
+                                          ADSC_OPT_PATH = 2 returns EINVAL.  Set it before adsc_bind. */
 
 #define ADSC_OPT_SPREAD              9  /* 1: latency mode for ensembles that do not fill the device: the resident path cuts
                                           every member into more, shorter CTAs (clusters of up to 8 CTAs of at least 256

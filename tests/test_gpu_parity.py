@@ -165,6 +165,75 @@ def test_cfg4_full_size_sampled(env):
     _bc_invariants(f)
 
 
+def test_cfg4_full_size_1000_steps(env, capsys):
+    """configs[3] as BASELINE.json states it: ONE member of N = 2^20+1 for 1000 RK4 steps ("Parity
+    runs: 1000 steps, all members for CFG 1/4"), in the launch configuration bench.py times (path 1, one chunk per
+    SM, 4000 stamped mailbox rounds in one launch), element by element against the oracle at the north_star
+    tolerance, with the end-point invariants and the diagnostics.  About five minutes of oracle time."""
+    import time
+    Phi, Pi, _ = env["inputs"].make("cfg4")
+    ens, f, d = _gpu_run(env, Phi, Pi, 1000)
+    assert ens.path[0] == 1 and ens.launch_count < 40        # one stepping launch, not one per step
+    t0 = time.time()
+    ev = env["oracle"].Evolution(Phi, Pi).step(1000)
+    el = time.time() - t0
+    worst = _compare(f, ev)
+    _bc_invariants(f)
+    od = ev.diagnostics()
+    assert d["steps_done"][0] == 1000 and d["collapsed"][0] == 0 and od["collapsed"][0] == 0
+    assert abs(d["mass"][0] - od["mass"][0]) <= 1e-12 * abs(od["mass"][0])
+    assert abs(d["min_A"][0] - od["min_A"][0]) <= TOL and d["argmin_A"][0] == od["argmin_A"][0]
+    assert abs(d["constraint_residual"][0] - od["resid"][0]) <= TOL
+    with capsys.disabled():
+        print("\n| cfg4 | N=%d | 1 member | 1000 steps | path %d (%d CTAs) | " % (Phi.shape[1], *ens.path)
+              + " | ".join("%s %.1e" % kv for kv in worst.items()) + " | oracle %.0f s |" % el)
+
+
+@pytest.mark.parametrize("order,path,name,B,N,nsteps", [
+    (3, 1, "cfg2", 2, 65537, 60),       # the paper's Table II size (N = 64K) with its production rule, persistent kernel
+    (3, 3, "cfg2", 2, 4097, 300),       # generic streaming kernels
+    (2, 1, "cfg5", 3, 2049, 301),
+    (3, 1, "cfg5", 3, 1033, 300),       # one ragged slice
+    (2, 3, "cfg5", 3, 1027, 300),       # N-1 = 2 mod 4
+    (3, 0, "cfg5", 4, 2049, 500),       # auto: no resident build of this combination, a streaming path takes it
+    (3, 0, "cfg5", 2, 1027, 200),
+])
+def test_fixed_background_rk_orders_match_oracle(env, order, path, name, B, N, nsteps):
+    """PAPER.md:57 (the paper's runs use the third-order rule) with PAPER.md:177 (Table II: A = 1, delta = 0 held
+    fixed): the fixed background under RK3 / RK2.  The resident kernel is not compiled for this combination; the
+    streaming kernels (stage count at run time) take it, also when the path is left on auto."""
+    Phi, Pi, _ = env["inputs"].make(name, B=B, N=N)
+    x = env["inputs"].grid(N)
+    Phi = Phi + 3.0 * np.sin(2 * x)[None, :] * np.cos(x)[None, :] ** 2
+    Phi[:, 0] = 0; Phi[:, -1] = 0
+    Pi = Pi * 20.0
+    ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=path, fixed_background=True, rk_order=order)
+    assert (ens.path[0] == path) if path else (ens.path[0] in (1, 3))
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 8), fixed_background=True, rk_order=order).step(nsteps)
+    scale = max(1.0, np.abs(ev.Pi).max())
+    for k, ref in (("Phi", ev.Phi), ("Pi", ev.Pi)):
+        assert np.isfinite(f[k]).all()
+        assert np.max(np.abs(f[k] - ref)) <= TOL * scale, (k, np.max(np.abs(f[k] - ref)))
+    assert (f["A"] == 1).all() and (f["delta"] == 0).all()
+    assert (f["Phi"][:, 0] == 0).all() and (f["Phi"][:, -1] == 0).all() and (f["Pi"][:, -1] == 0).all()
+    assert (d["steps_done"] == nsteps).all() and (d["collapsed"] == 0).all()
+    # not RK4 in disguise: on the coarser grids (where dt is large enough for the rules to differ visibly) the
+    # fourth-order evolution of the same data is much further from the oracle's RK3 / RK2 result than the GPU is
+    if N < 3000:
+        ev4 = env["oracle"].Evolution(Phi, Pi, nthreads=min(B, 8), fixed_background=True).step(nsteps)
+        gpu_err = max(np.max(np.abs(f[k] - ref)) for k, ref in (("Phi", ev.Phi), ("Pi", ev.Pi)))
+        assert np.max(np.abs(ev4.Pi - ev.Pi)) > 100 * max(gpu_err, 1e-13), (np.max(np.abs(ev4.Pi - ev.Pi)), gpu_err)
+    if path == 0:
+        binding = env["binding"]
+        lib = binding.load_library()
+        h = lib.adsc_create(N, B, 0.25, 0.1)
+        assert lib.adsc_set_option(h, binding.ADSC_OPT_FIXED_BACKGROUND, 1.0) == 0
+        assert lib.adsc_set_option(h, binding.ADSC_OPT_RK_ORDER, float(order)) == 0
+        assert lib.adsc_set_option(h, binding.ADSC_OPT_PATH, 2.0) == binding.ADSC_EINVAL     # no resident build: said, not hidden
+        assert lib.adsc_path(h, None) in (1, 3)
+        lib.adsc_destroy(h)
+
+
 @pytest.mark.parametrize("N,path", [(9, 1), (17, 1), (33, 1), (129, 2), (1001, 1), (257, 2), (513, 1), (17, 3), (1001, 3),
                                     (1027, 3), (2051, 3), (249, 1), (265, 1), (1793, 1), (2057, 1), (7177, 1), (7169, 1),
                                     (14345, 1), (1027, 1), (2051, 1)])
