@@ -78,6 +78,11 @@ def parse():
     ap.add_argument("--mode-energies", type=int, default=0, metavar="J",
                     help="also time adsc_mode_energies(J) (SURVEY.md 8(f) f3) on the evolved ensemble and add a "
                          "`mode_energies` object with its own roofline to the line")
+    ap.add_argument("--extra-workloads", default="cfg3,cfg5,cfg4,paper32k:1", metavar="LIST",
+                    help="comma list of name[:path] also timed at N=1 (device-resident, own roofline) and reported in "
+                         "`workloads`: the other configs the 60 %% target is stated on, cfg4, and the paper's "
+                         "production shape forced onto the streaming kernel (the one workload that leaves L2); '' = none")
+    ap.add_argument("--extra-seconds", type=float, default=1.0, help="timed window of each extra workload")
     ap.add_argument("--probe-ms", type=float, default=50.0, help="duration of each roofline-denominator probe (0 = skip)")
     a = ap.parse_args()
     if a.rk_order == 0:
@@ -198,6 +203,101 @@ def fast_build_rate(name, N, seconds, fixed, rk_order):
         return {"value": None, "error": str(e)[:200]}
     finally:
         oracle.use_build("oracle")
+
+
+def make_roofline(path, B, N, NS, fixed, per_gpu_rate, rk4, launches_per_step, probe, peaks, probe_ms):
+    """The `roofline` object of one workload on one GPU: resident path = FP64 ALU bound,
+    streaming paths = the [NS] HBM line with the ALU fraction beside it."""
+    peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
+    slots = (SLOTS_PER_POINT_STEP_FIXED if fixed else SLOTS_PER_POINT_STEP) * NS / 4.0
+    ach_tf = per_gpu_rate * slots * 2 / 1e12
+    peak_src = (f"derived: {N_SMS} SMs x {FP64_LANES_PER_SM} DFMA lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 flop "
+                f"(DESIGN.md Roofline); peak_measured: adsc_probe(FP64_FMA) run for {probe_ms:.0f} ms before "
+                f"the timed region")
+    fp64_meas = probe["fp64_fma_tflops"] if probe else None
+    if path == 2:
+        return {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": ach_tf / peak_tf,
+                "peak_measured": fp64_meas, "frac_of_measured": (ach_tf / fp64_meas) if fp64_meas else None,
+                "shared_load_tbs_measured": probe["shared_load_tbs"] if probe else None,
+                "traffic": 6.0 * B * N * 8,
+                "traffic_unit": "global-memory bytes per launch: the three fields are loaded once and stored once, whatever "
+                                "the number of steps in the launch (the ncu dram figures are in profiles/)",
+                "kernel": f"k_resident3 (whole RK steps on chip; {launches_per_step} launch per adsc_step)",
+                "peak_src": peak_src,
+                "algorithmic": f"{slots:.0f} FP64-pipe instr per point per step"}
+    # [NS]/SURVEY.md 8(d) streaming roofline: bytes per point per step with one fused pass per stage:
+    # first and last stage 72 B, every middle stage 120 B
+    bytes_step = 72.0 * 2 + 120.0 * (NS - 2)
+    if fixed:
+        bytes_step *= 2.0 / 3.0                       # two evolved fields instead of three
+    ach = per_gpu_rate * bytes_step / 1e9
+    kern_bytes = (STREAM_BYTES_STAGE_FIRST + STREAM_BYTES_STAGE_LAST + STREAM_BYTES_STAGE_MID * (NS - 2)
+                  + STREAM_BYTES_TABLES * NS)
+    wset = 9.0 * B * N * 8 + 3.0 * N * 8
+    return {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+            "frac": ach / peaks["hbm_gbs"],
+            "traffic": (kern_bytes * rk4 + 48.0) * B * N if path == 1 else None,
+            "traffic_unit": "global-memory bytes per launch the kernel provably requests (u^n, accumulator, tables; "
+                            "load + store of the fields once); see l2_resident",
+            "kernel_bytes_per_point_step": kern_bytes if path == 1 else None,
+            "working_set_bytes": wset, "l2_resident": bool(wset < L2_BYTES),
+            "alu": {"achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
+                    "peak_measured": fp64_meas, "frac_of_measured": (ach_tf / fp64_meas) if fp64_meas else None},
+            "note": ("the [NS] streaming roofline (algorithmic bytes over the HBM copy peak); when l2_resident is true "
+                     "the working set never leaves the 126 MB L2, HBM is not the binding resource and the `alu` "
+                     "fraction is the one that measures the kernel"),
+            "kernel": ("k_stream_async (stage state in shared memory, tables staged by cp.async.bulk rings, "
+                       "u^n/accumulator through L2; 1 cooperative launch per adsc_step)" if path == 1 else
+                       "k_stream_rhs (+ k_stream_I, k_stream_carry: 3 launches per RK stage)"),
+            "peak_src": f"{peaks['src']} copy bandwidth (MEASURED_PEAKS.json); alu: " + peak_src,
+            "algorithmic": f"{bytes_step:.0f} B per point per step"}
+
+
+def time_extra_workload(torch, binding, inputs, dev, index, flush, name, path_opt, seconds, probe, peaks, probe_ms):
+    """One more BASELINE.json config (or the paper's production shape) at full size on this GPU, by the protocol of the
+    headline: 3 warm-up adsc_step calls, then enough calls for >= `seconds` of device time, L2 flushed before each,
+    CUDA events on the stream the kernels run on, clocks sampled during the window.  Device-resident only (no e2e,
+    no CPU leg: those belong to the headline workload)."""
+    cfg = inputs.CONFIGS[name]
+    N, B = cfg["N"], cfg["B"]
+    order = 3 if name == "paper32k" else 4
+    rk4 = RK4_PER_STEP[name]
+    Phi, Pi, _ = inputs.make(name, B=B, N=N)
+    ens = binding.Ensemble(N, B, device=dev, path=path_opt, rk_order=(order if order != 4 else None))
+    path, cluster = ens.path
+    ens.set_initial(torch.from_numpy(np.ascontiguousarray(Phi)).to(dev), torch.from_numpy(np.ascontiguousarray(Pi)).to(dev))
+    del Phi, Pi
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ms1 = 0.0
+    for _ in range(3):                                           # warm-up (the last one also sizes the window)
+        a.record(); ens.step(rk4); b.record(); torch.cuda.synchronize(dev)
+        ms1 = a.elapsed_time(b)
+    K = max(3, min(40, int(np.ceil(seconds * 1e3 / max(ms1, 1e-3)))))
+    l0 = ens.launch_count
+    sampler = ClockSampler(index)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    t0 = time.time()
+    for a, b in evs:
+        flush.fill_(1)
+        a.record(); ens.step(rk4); b.record()
+    torch.cuda.synchronize(dev)
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    launches = ens.launch_count - l0
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    d = ens.diagnostics()
+    value = float(B) * N * rk4 * K / (ms * 1e-3)
+    out = {"workload": WORKLOAD_DESC[name], "name": name, "N": N, "batch": B, "rk_order": order, "rk_steps_per_step": rk4,
+           "path": {1: "streaming-persistent", 2: "resident", 3: "streaming-generic"}[path], "ctas_per_member": cluster,
+           "value": value, "unit": UNIT, "steps": K, "warmup": 3, "ms_per_step": ms / K, "timed_region_s": ms * 1e-3,
+           "active_fraction": float((d["collapsed"] == 0).mean()), "gpu_launches": int(launches),
+           "roofline": make_roofline(path, B, N, order, False, value, rk4, launches // K, probe, peaks, probe_ms),
+           "clocks": clocks}
+    ens.close()
+    del ens
+    torch.cuda.empty_cache()
+    return out
 
 
 # ----------------------------------------------------------------------------- reference arm
@@ -388,53 +488,21 @@ def main():
         return 0
 
     peaks = load_peaks()
-    per_gpu_rate = value / world
-    NS = args.rk_order
-    peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
-    slots = (SLOTS_PER_POINT_STEP_FIXED if args.fixed_background else SLOTS_PER_POINT_STEP) * NS / 4.0
-    ach_tf = per_gpu_rate * slots * 2 / 1e12
-    peak_src = (f"derived: {N_SMS} SMs x {FP64_LANES_PER_SM} DFMA lanes x {peaks['sm_max_mhz']:.0f} MHz x 2 flop "
-                f"(DESIGN.md Roofline); peak_measured: adsc_probe(FP64_FMA) run for {args.probe_ms:.0f} ms before "
-                f"the timed region")
-    fp64_meas = probe["fp64_fma_tflops"] if probe else None
-    if path == 2:
-        roof = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach_tf / peak_tf,
-                "peak_measured": fp64_meas, "frac_of_measured": (ach_tf / fp64_meas) if fp64_meas else None,
-                "shared_load_tbs_measured": probe["shared_load_tbs"] if probe else None,
-                "traffic": 6.0 * B * N * 8,
-                "traffic_unit": "global-memory bytes per launch: the three fields are loaded once and stored once, whatever "
-                                "the number of steps in the launch (the ncu dram figures are in profiles/)",
-                "kernel": f"k_resident3 (whole RK steps on chip; {launches // max(K, 1)} launch per adsc_step)",
-                "peak_src": peak_src,
-                "algorithmic": f"{slots:.0f} FP64-pipe instr per point per step"}
-    else:
-        # [NS]/SURVEY.md 8(d) streaming roofline: bytes per point per step with one fused pass per stage:
-        # first and last stage 72 B, every middle stage 120 B
-        bytes_step = 72.0 * 2 + 120.0 * (NS - 2)
-        if args.fixed_background:
-            bytes_step *= 2.0 / 3.0                       # two evolved fields instead of three
-        ach = per_gpu_rate * bytes_step / 1e9
-        kern_bytes = (STREAM_BYTES_STAGE_FIRST + STREAM_BYTES_STAGE_LAST + STREAM_BYTES_STAGE_MID * (NS - 2)
-                      + STREAM_BYTES_TABLES * NS)
-        wset = 9.0 * B * N * 8 + 3.0 * N * 8
-        roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"],
-                "traffic": (kern_bytes * rk4 + 48.0) * B * N if path == 1 else None,
-                "traffic_unit": "global-memory bytes per launch the kernel provably requests (u^n, accumulator, tables; "
-                                "load + store of the fields once); see l2_resident",
-                "kernel_bytes_per_point_step": kern_bytes if path == 1 else None,
-                "working_set_bytes": wset, "l2_resident": bool(wset < L2_BYTES),
-                "alu": {"achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
-                        "peak_measured": fp64_meas, "frac_of_measured": (ach_tf / fp64_meas) if fp64_meas else None},
-                "note": ("the [NS] streaming roofline (algorithmic bytes over the HBM copy peak); when l2_resident is true "
-                         "the working set never leaves the 126 MB L2, HBM is not the binding resource and the `alu` "
-                         "fraction is the one that measures the kernel"),
-                "kernel": ("k_stream_async (stage state in shared memory, tables staged by cp.async.bulk rings, "
-                           "u^n/accumulator through L2; 1 cooperative launch per adsc_step)" if path == 1 else
-                           "k_stream_rhs (+ k_stream_I, k_stream_carry: 3 launches per RK stage)"),
-                "peak_src": f"{peaks['src']} copy bandwidth (MEASURED_PEAKS.json); alu: " + peak_src,
-                "algorithmic": f"{bytes_step:.0f} B per point per step"}
+    roof = make_roofline(path, B, N, args.rk_order, args.fixed_background, value / world, rk4, launches // max(K, 1),
+                         probe, peaks, args.probe_ms)
+
+    # ---- the other configs the north_star target is stated on, by the same protocol, each with its own roofline
+    extra = None
+    if args.extra_workloads and world == 1:
+        del ens, pe, Phi_d, Pi_d, Phi_h, Pi_h, Phi_o, Pi_o, A_o, out
+        torch.cuda.empty_cache()
+        extra = []
+        for spec in args.extra_workloads.split(","):
+            wname, _, wpath = spec.partition(":")
+            if wname == name and int(wpath or 0) == args.path:
+                continue
+            extra.append(time_extra_workload(torch, binding, inputs, dev, local_rank, flush, wname, int(wpath or 0),
+                                             args.extra_seconds, probe, peaks, args.probe_ms))
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
@@ -463,7 +531,10 @@ def main():
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if extra is not None:
+        line["workloads"] = extra
     if modes is not None:
+        peak_tf = N_SMS * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 * 2 / 1e12
         modes["roofline"] = {"bound": "alu", "achieved": modes.pop("achieved_tflops"), "peak": peak_tf, "unit": "TFLOP/s"}
         modes["roofline"]["frac"] = modes["roofline"]["achieved"] / peak_tf
         line["mode_energies"] = modes
