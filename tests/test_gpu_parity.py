@@ -745,6 +745,52 @@ def test_bitwise_reproducible(env, N, B, path):
             assert np.array_equal(o[k], outs[0][k]), k
 
 
+@pytest.mark.parametrize("N,B,path", [(20481, 40, 1), (2 ** 18 + 1, 2, 1), (32769, 40, 1), (32769, 12, 2)])
+def test_bitwise_reproducible_under_contention(env, N, B, path):
+    """Ten repetitions of the same launch, nine of them with other kernels running beside it on a second stream for the
+    whole launch (memory-bound fills and FP64 matrix products: they take SMs, L2 and DRAM bandwidth away at changing
+    moments), all bit-identical to the undisturbed first one.  The stamped-mailbox and table-ring protocols of the
+    persistent streaming kernel and the DSMEM exchange of the 16-CTA clusters rest on ordering assumptions
+    ("mailbox assumption") that no sanitizer can check on this pool: a torn slot or a reordered refill
+    shows up as a run-to-run difference."""
+    torch = env["torch"]
+    Phi, Pi, _ = env["inputs"].make("cfg2", B=B, N=N)
+    Pi = Pi * 3.0
+    side = torch.cuda.Stream()
+    buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    m = torch.randn(1024, 1024, dtype=torch.float64, device="cuda")
+    binding = env["binding"]
+    dPhi, dPi = torch.from_numpy(Phi).cuda(), torch.from_numpy(Pi).cuda()
+    first = None
+    for rep in range(10):
+        ens = binding.Ensemble(N, B, path=path)
+        assert ens.path[0] == path
+        ens.set_initial(dPhi, dPi)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]      # side start / end, step start / end
+        if rep:
+            with torch.cuda.stream(side):                   # tens of ms of other work, enqueued just ahead of the launch
+                ev[0].record()
+                for k in range(150 + 30 * rep):
+                    buf.fill_(k & 255)
+                    if k % 3 == rep % 3:
+                        m = (m @ m) * 1e-3
+                ev[1].record()
+        ev[2].record()
+        ens.step(24)                                        # a few ms
+        ev[3].record()
+        torch.cuda.synchronize()
+        if rep:                                             # the step ran inside the side stream's busy window
+            assert ev[0].elapsed_time(ev[2]) >= 0.0 and ev[3].elapsed_time(ev[1]) > 0.0, \
+                (ev[0].elapsed_time(ev[2]), ev[3].elapsed_time(ev[1]))
+        f = {k: v.cpu().numpy() for k, v in ens.get_fields().items()}
+        if first is None:
+            first = f
+            continue
+        for k in ("Phi", "Pi", "A", "delta"):
+            assert np.array_equal(f[k], first[k]), (rep, k)
+
+
 def test_roofline_probes_are_plausible(env):
     """adsc_probe (the denominators bench.py reports as measured): FP64 FMA rate below the derived peak of the device
     and above half of it; conflict-free 128-bit shared-memory loads between 64 and 128 B per clock and SM."""
