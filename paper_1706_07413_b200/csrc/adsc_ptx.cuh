@@ -62,17 +62,18 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void *src_glob
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst_smem), "l"(src_global), "r"(bytes), "r"(mbar) : "memory");
 }
-// The same for a buffer the issuing warp has just READ with ordinary shared-memory loads (a ring slot that is being
-// refilled).  The copy engine is not ordered behind the load/store queue: a bulk copy issued right after the loads can
-// land before a queued load has executed.  mbarrier.arrive is queued behind the warp's earlier loads, and the copy is
-// made to depend on the state token it returns, so the copy cannot be issued before those loads have read the slot.
-__device__ __forceinline__ void bulk_g2s_after_reads(uint32_t dst_smem, const void *src_global, uint32_t bytes, uint32_t mbar)
+// mbarrier.arrive.expect_tx followed by the bulk copy that completes it (one thread).
+__device__ __forceinline__ void bulk_g2s_arrive(uint32_t dst_smem, const void *src_global, uint32_t bytes, uint32_t mbar)
 {
-    asm volatile("{\n\t.reg .b64 st;\n\t.reg .pred p;\n\t"
-                 "mbarrier.arrive.expect_tx.shared::cta.b64 st, [%3], %2;\n\t"
-                 "setp.ne.b64 p, st, 0xffffffffffffffff;\n\t"
-                 "@p cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n\t}"
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%3], %2;\n\t"
+                 "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst_smem), "l"(src_global), "r"(bytes), "r"(mbar) : "memory");
+}
+// Orders this thread's earlier generic-proxy accesses to shared memory (and those a preceding warp barrier made
+// cumulative) before its later async-proxy operations (bulk copies into the same buffer).
+__device__ __forceinline__ void fence_proxy_async_smem()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 // 256-bit global accesses (sm_100: LDG.E.256 / STG.E.256), 32-byte aligned.
 __device__ __forceinline__ void ldg256(const double *p, double &a, double &b, double &c, double &d)

@@ -88,7 +88,6 @@ struct SAParams {
     long long nsteps;
     int check_last;
     int G, groups, SQ;               // chunks per member, concurrent members, slices per chunk
-    unsigned zero;                   // 0, but unknown to the compiler (see ring_next)
     SAConsts k;
 };
 
@@ -217,26 +216,36 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
     // keeps its tables for the whole launch.
     unsigned phs = 0;                                    // phase parities: bits 0..2 ring slots, 3 mbF, 4 mbC
     const bool reload = n_my > 1;
-    auto ring_issue = [&](int t, int qn, unsigned dep) {
-        if (lane == 0) {
-            bulk_g2s_after_reads(ringw + t * SA_SLOT, prm.tabp + ((size_t)(cs0 + qn) * 3 + t) * SA_SL,
-                                 SA_SLOT + (dep & prm.zero), mbR + 8 * t);
-        }
+    auto ring_issue = [&](int t, int qn) {               // first fill: nobody has read the slot yet
+        if (lane == 0)
+            bulk_g2s_arrive(ringw + t * SA_SLOT, prm.tabp + ((size_t)(cs0 + qn) * 3 + t) * SA_SL, SA_SLOT, mbR + 8 * t);
     };
     if (n_my > 0) {
         const int q0 = SA_NW * (n_my - 1) + warp;
-        if (!FIXED) ring_issue(0, q0, 0u);
-        ring_issue(1, q0, 0u); ring_issue(2, q0, 0u);
+        if (!FIXED) ring_issue(0, q0);
+        ring_issue(1, q0); ring_issue(2, q0);
     }
     auto ring_wait = [&](int t) { mbar_wait<false>(mbR + 8 * t, (phs >> t) & 1u); };
-    // After the warp has read slot t of slice q (tile j): fetch the same table of its next slice.  The copy engine is
-    // not ordered behind the warp's shared-memory loads, so the copy is made to DEPEND on them: `dep` mixes one word of
-    // every load of the slot into the byte count (and with a run-time zero), and the copy is predicated on the state
-    // token of the mbarrier arrive (adsc_ptx.cuh).  Without this a queued load could read the NEXT slice's table.
-    auto ring_next = [&](int t, int j, unsigned dep) {
+    // After the warp has read slot t of slice q (tile j): fetch the same table of its next slice.  The copy engine
+    // (async proxy) is not ordered behind the warp's shared-memory loads (generic proxy): without an explicit order a
+    // queued load could read the NEXT slice's table (seen in round 2 as a run-to-run difference).  The documented
+    // order: __syncwarp (every lane's loads of the slots are done and cumulative to lane 0), then
+    // fence.proxy.async.shared::cta in the issuing lane, then arrive + copy.  One warp barrier and one proxy fence per
+    // slice serve all three slots: their refills are issued together once the last table (t = 2) has been read; the
+    // warp's next slice starts long after that.  (Round 2 ordered each refill by predicating the copy on the arrive
+    // token and making its byte count data-dependent on the loaded words -- instruction-issue order, which PTX does not
+    // promise; the fenced form is also 3 % faster on cfg4, 5 % on paper32k.)
+    auto ring_next = [&](int t, int j) {
         if (reload) {
-            // (lane 0's words are enough: a load is one warp instruction, its registers are released together)
-            ring_issue(t, SA_NW * (j > 0 ? j - 1 : n_my - 1) + warp, dep);
+            if (t == 2) {
+                const int qn = SA_NW * (j > 0 ? j - 1 : n_my - 1) + warp;
+                __syncwarp();
+                if (lane == 0) {
+                    fence_proxy_async_smem();
+                    for (int u = FIXED ? 1 : 0; u < 3; ++u)
+                        bulk_g2s_arrive(ringw + u * SA_SLOT, prm.tabp + ((size_t)(cs0 + qn) * 3 + u) * SA_SL, SA_SLOT, mbR + 8 * u);
+                }
+            }
             phs ^= 1u << t;
         }
     };
@@ -500,8 +509,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         for (int k = 0; k < 4; ++k) { const double2 m = slot[k * 32 + lane]; m2[2 * k] = m.x; m2[2 * k + 1] = m.y; }
                         const double scm = (lane == 0) ? esc[2 * q] : slot[3 * 32 + lane - 1].y;
                         const double scp = (lane == 31) ? esc[2 * q + 1] : slot[lane + 1].x;
-                        ring_next(0, j, (unsigned)(__double2hiint(m2[0]) | __double2hiint(m2[2]) | __double2hiint(m2[4]) | __double2hiint(m2[6])
-                                                   | __double2hiint(scm) | __double2hiint(scp)));
+                        ring_next(0, j);
                         fm = scm * fma(hlP[2], hlP[2], hlQ[2] * hlQ[2]);          // f'_{-1}
                         fp = scp * fma(hrP[0], hrP[0], hrQ[0] * hrQ[0]);          // f'_{P}
                     }
@@ -569,7 +577,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         double tT[P];
 #pragma unroll
                         for (int k = 0; k < 4; ++k) { const double2 m = slot[128 + k * 32 + lane]; tT[2 * k] = m.x; tT[2 * k + 1] = m.y; }
-                        ring_next(1, j, (unsigned)(__double2hiint(tT[0]) | __double2hiint(tT[2]) | __double2hiint(tT[4]) | __double2hiint(tT[6])));
+                        ring_next(1, j);
                         // the stage state is read again (it is still unchanged in shared memory) rather than kept in
                         // registers across the exponentials
 #pragma unroll
@@ -599,10 +607,13 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                         mbar_wait<false>(mbC, cpar);
                         Cst = scal[1];
                         if (s == 0 && n > 0 && scal[0] != 0.0) {                  // a6: nothing has been changed yet
-                            if (reload) {                                         // the ring is ahead by one slice: put it back
-                                const int q0 = SA_NW * (n_my - 1) + warp;
-                                ring_wait(0); ring_issue(0, q0, 0u); phs ^= 1u;
-                                ring_wait(1); ring_issue(1, q0, 0u); phs ^= 2u;
+                            if (reload) {
+                                // Slots 0 and 1 have been read and their phase bits advanced, but no refill has been
+                                // issued yet (ring_next issues all three behind the read of slot 2, which is still
+                                // ahead): the ring still holds this first slice's tables, which is what the next
+                                // member starts with.  Take the two phase bits back.
+                                if (!FIXED) phs ^= 1u;
+                                phs ^= 2u;
                             }
                             collapsed = 1;
                             break;
@@ -666,7 +677,7 @@ __global__ void __launch_bounds__(SA_T, 1) k_stream_async(const __grid_constant_
                     ring_wait(2);
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const double2 m = slot[256 + k * 32 + lane]; tC[2 * k] = m.x; tC[2 * k + 1] = m.y; }
-                    ring_next(2, j, (unsigned)(__double2hiint(tC[0]) | __double2hiint(tC[2]) | __double2hiint(tC[4]) | __double2hiint(tC[6])));
+                    ring_next(2, j);
                     const double d4cC = K.d4c * Cl;
                     if (defer) {
 #pragma unroll
@@ -853,7 +864,7 @@ cudaError_t launch_stream_async(adsc_ctx *c, long long nsteps, int check_last)
     prm.tabp = c->ws.tabp;
     prm.rec = c->ws.rec; prm.mbox = c->ws.sp_mbox;
     prm.nsteps = nsteps; prm.check_last = check_last;
-    prm.G = c->sp_G; prm.groups = c->sp_groups; prm.SQ = c->sp_SQ; prm.zero = 0u;
+    prm.G = c->sp_G; prm.groups = c->sp_groups; prm.SQ = c->sp_SQ;
     {
         const double h = c->pb.h, dt = c->pb.dt, koc = c->pb.ko_eps / (64.0 * h);
         SAConsts &k = prm.k;

@@ -288,6 +288,35 @@ def test_collapse_flags_and_times(env, path):
             assert np.max(np.abs(f[k][b] - ref[b])) <= 1e-9 * scale, (b, k)
 
 
+@pytest.mark.parametrize("N,B,order", [(20481, 120, 4), (40961, 30, 3)])
+def test_collapse_on_long_streaming_chunks(env, N, B, order):
+    """Collapse on the persistent streaming kernel when a warp owns several slices of its chunk (chunks of more than
+    2048 points: the table ring is being refilled when the collapse is seen and has to be left in the state the next
+    member of the same CTA group expects), with more members than concurrent groups so that every group goes on to
+    further members after a collapsed one.  Every third member is forced to collapse at the first check."""
+    Phi, Pi, _ = env["inputs"].make("cfg2", B=B, N=N)
+    Pi[::3] *= 1.0e3
+    nsteps = 24
+    ens, f, d = _gpu_run(env, Phi, Pi, nsteps, path=1, rk_order=order)
+    assert ens.path[0] == 1 and (N - 1) // ens.path[1] > 2048 and B > 148 // ens.path[1]
+    ev = env["oracle"].Evolution(Phi, Pi, nthreads=16, rk_order=order).step(nsteps)
+    od = ev.diagnostics()
+    assert od["collapsed"][::3].all() and not od["collapsed"][1::3].any() and not od["collapsed"][2::3].any()
+    assert (d["collapsed"] == od["collapsed"]).all() and (d["steps_done"] == od["steps_done"]).all()
+    live = np.where(od["collapsed"] == 0)[0]
+    for k, ref in (("Phi", ev.Phi), ("Pi", ev.Pi), ("A", ev.A), ("delta", ev.delta)):
+        assert np.max(np.abs(f[k][live] - ref[live])) <= TOL, k
+    for b in np.where(od["collapsed"] == 1)[0]:
+        assert abs(d["t_collapse"][b] - od["t_collapse"][b]) <= ev.dt * 1e-9
+    # and once more in a second call on the same handle: the frozen members stay frozen, the others go on
+    ens.step(nsteps)
+    ev.step(nsteps)
+    f2 = {k: v.cpu().numpy() for k, v in ens.get_fields().items()}
+    for k, ref in (("Phi", ev.Phi), ("Pi", ev.Pi), ("A", ev.A)):
+        assert np.max(np.abs(f2[k][live] - ref[live])) <= TOL, k
+    assert (ens.diagnostics()["steps_done"] == ev.diagnostics()["steps_done"]).all()
+
+
 def test_frozen_member_is_not_advanced(env):
     Phi, Pi, _ = env["inputs"].make("tcollapse", B=8)
     torch, binding = env["torch"], env["binding"]
